@@ -1,0 +1,378 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (pins P2-P11).
+
+None of these compares the oracle with itself or with the CUDA path: expected values are the spec's
+big-int vectors (tests/golden/), plain string manipulation, closed forms, invariants and brute force.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import seqgen
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+BASES = "ACGT"
+
+
+def pack_str(s):
+    v = 0
+    for c in s:
+        v = (v << 2) | BASES.index(c)
+    return v
+
+
+# ---------------------------------------------------------------- P11: hash vectors
+def test_p11_hash_vectors():
+    n = 0
+    for line in open(os.path.join(GOLD, "hash_vectors.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        lhs, rhs = line.split("=")
+        name, *args = lhs.split()
+        args = [int(a, 0) for a in args]
+        want = int(rhs.strip(), 0)
+        got = {"g": lambda m, x: oracle.g(m, x), "sigma": lambda key, P: oracle.sigma(key, P),
+               "f": lambda s, x: oracle.f(s, x), "bitpos": lambda h, i, H: oracle.bitpos(h, i, H)}[name](*args)
+        assert got == want, line
+        n += 1
+    assert n == 16
+
+
+def test_bitpos_slices_and_fallback():
+    h = 0xFEDCBA9876543210
+    # A5: W = floor(64/H), slice i starts at bit i*W, low 6 bits of the slice
+    for H in (1, 2, 3, 4, 5, 6, 7, 8, 9, 10):
+        W = 64 // H
+        for i in range(H):
+            assert oracle.bitpos(h, i, H) == (h >> (i * W)) & 63
+    # A6: H > 10 -> top 6 bits of h * ((2i+1) * golden) mod 2^64
+    for H in (11, 12, 16):
+        for i in range(H):
+            salt = ((2 * i + 1) * 0x9E3779B97F4A7C15) & ((1 << 64) - 1)
+            assert oracle.bitpos(h, i, H) == ((h * salt) & ((1 << 64) - 1)) >> 58
+
+
+def test_code_alphabet_a9():
+    for c, v in zip("ACGTacgt", [0, 1, 2, 3] * 2):
+        assert oracle.code(c) == v
+    for c in range(256):
+        if chr(c) not in "ACGTacgt":
+            assert oracle.code(c) == -1
+
+
+# ---------------------------------------------------------------- P10: Fig. 2 worked example
+def test_p10_fig2_window_enumeration():
+    lines = [l.strip() for l in open(os.path.join(GOLD, "fig2_windows.txt")) if l.strip() and not l.startswith("#")]
+    _, S, k, m, s = lines[0].split()
+    k, m, s = int(k), int(m), int(s)
+    o = oracle.OracleSBF(k, m, s, 4, 1 << 12)
+    kmers = [l for l in lines if l.startswith("kmer")]
+    assert len(kmers) == len(S) - k + 1 == 4
+    common = None
+    for l in kmers:
+        head, mm, ss = [x.split() for x in l.split("|")]
+        p, kmer = int(head[1]), head[2]
+        assert S[p:p + k] == kmer
+        v = o.pack_kmer(S, p)
+        assert v == pack_str(kmer)
+        assert len(mm) == k - m + 1 == 5 and len(ss) == k - s + 1 == 4
+        for i, x in enumerate(mm):
+            assert oracle.sub(v, k, i, m) == pack_str(x)
+        for j, x in enumerate(ss):
+            assert oracle.sub(v, k, j, s) == pack_str(x)
+        # the oracle's minimizer is one of the k-mer's own m-mers, namely the one with the least key
+        keys = [oracle.g(m, pack_str(x)) for x in mm]
+        assert o.min_key(v) == min(keys)
+        common = set(mm) if common is None else common & set(mm)
+    assert common == set(lines[-1].split()[1:]) == {"GAAAC", "AAACT"}
+    assert o.pack_kmer(S, len(S) - k + 1) is None          # runs off the end: no k-mer
+
+
+# ---------------------------------------------------------------- P1: window minimum vs naive scan over string m-mers
+@pytest.mark.parametrize("k,m", [(31, 16), (31, 12), (31, 20), (21, 11), (32, 32), (9, 5)])
+def test_p1_min_key_is_window_minimum(k, m):
+    rng = np.random.default_rng(5)
+    seqs = ["".join(rng.choice(list(BASES), 400)), "A" * 200, "AC" * 100, "ACGT" * 50 + "T" * 60]
+    o = oracle.OracleSBF(k, m, min(k, 28), 4, 1 << 14)
+    for S in seqs:
+        # key of every m-mer, extracted from the string (not through sbfo_sub)
+        mkeys = np.array([oracle.g(m, pack_str(S[i:i + m])) for i in range(len(S) - m + 1)], dtype=np.uint64)
+        mk, _, valid = o.trace(S)
+        w = k - m + 1
+        for p in range(len(S) - k + 1):
+            assert valid[p] and mk[p] == mkeys[p:p + w].min()
+        assert not valid[len(S) - k + 1:].any()
+
+
+# ---------------------------------------------------------------- P2: density 2/(w+1)
+@pytest.mark.parametrize("m,density", [(16, 2 / 17), (12, 2 / 21), (20, 2 / 13)])
+def test_p2_minimizer_density(m, density):
+    k = 31
+    seq = seqgen.uniform(101, 2_000_000)
+    o = oracle.OracleSBF(k, m, 28, 4, 1 << 20)
+    mk, _, valid = o.trace(seq)
+    n = seq.size - k + 1
+    assert valid[:n].all()
+    runs = 1 + np.count_nonzero(mk[1:n] != mk[:n - 1])
+    got = runs / n
+    # d ~ 2/(w+1); mean super-k-mer length (w+1)/2 = 8.5 at m=16
+    assert abs(got / density - 1) < 0.01, (got, density)
+
+
+# ---------------------------------------------------------------- P3: shard uniformity
+def test_p3_shard_uniformity():
+    k = 31
+    seq = seqgen.uniform(102, 6_000_000)
+    o = oracle.OracleSBF(k, 16, 28, 4, 1 << 20)     # P = 12
+    assert o.num_shards == 4096
+    mk, sh, valid = o.trace(seq)
+    n = seq.size - k + 1
+    head = np.ones(n, dtype=bool)
+    head[1:] = mk[1:n] != mk[:n - 1]
+    # k-mer load of the lower vs upper half of the shard range (same split for any P: top bit of sigma)
+    lower = np.count_nonzero(sh[:n] < 2048)
+    assert abs(lower / (n - lower) - 1) < 0.01
+    # one count per super-k-mer: chi-square over the 4096 shards
+    cnt = np.bincount(sh[:n][head].astype(np.int64), minlength=4096)
+    exp = cnt.sum() / 4096
+    chi2 = ((cnt - exp) ** 2 / exp).sum() / 4095
+    assert 0.9 < chi2 < 1.1, chi2
+    # sigma's P-dependence: sigma(key, P) is the top P bits of sigma(key, 32)
+    for key in (0, 1, 0xB524331D, 0xFFFFFFFF, 12345):
+        full = oracle.sigma(key, 32)
+        for P in (0, 1, 12, 27, 32):
+            assert oracle.sigma(key, P) == full >> (32 - P)
+
+
+# ---------------------------------------------------------------- P4: no false negatives, invalid -> false
+def test_p4_no_false_negatives_and_validity():
+    k = 31
+    seq = seqgen.uniform(7, 30_000).copy()
+    seq[5000:5100] = ord("N")
+    seq[12_345] = ord("n")
+    seq[20_000] = ord("R")            # IUPAC code: invalid (A9)
+    seq[100:200] = np.frombuffer(bytes(seq[100:200]).lower(), dtype=np.uint8)   # lower case is valid
+    offsets = np.array([0, 10, 10, 7000, 7030, 7061, 30_000], dtype=np.uint64)  # short, empty, long, k-1, k, long
+    o = oracle.OracleSBF(k, 16, 28, 4, 1 << 22)
+    nv = o.insert_records(seq, offsets)
+    bitmap, counts, nv2 = o.query_records(seq, offsets)
+    bits = oracle.bitmap_bits(bitmap, seq.size)
+    # expected validity straight from the text
+    ok_sym = np.isin(seq, np.frombuffer(b"ACGTacgt", dtype=np.uint8))
+    expect = np.zeros(seq.size, dtype=bool)
+    for r in range(len(offsets) - 1):
+        a, b = int(offsets[r]), int(offsets[r + 1])
+        for p in range(a, b - k + 1):
+            expect[p] = ok_sym[p:p + k].all()
+    assert nv == nv2 == expect.sum() == o.count_valid_kmers(seq, offsets)
+    assert (bits == expect).all()                      # every inserted k-mer true, everything else 0
+    assert counts.tolist() == [int(expect[int(offsets[r]):int(offsets[r + 1])].sum()) for r in range(6)]
+    assert counts[0] == counts[1] == counts[3] == 0 and counts[4] == 1
+    # case-insensitive: the lower-case copy of a k-mer is the same k-mer
+    assert o.pack_kmer(seq, 120) == o.pack_kmer(np.frombuffer(bytes(seq).upper(), dtype=np.uint8), 120)
+
+
+# ---------------------------------------------------------------- P5: brute force against the exact k-mer set
+@pytest.mark.parametrize("k,m,s,H", [(31, 16, 28, 4), (15, 8, 12, 2), (9, 5, 6, 4), (20, 20, 20, 3), (32, 16, 31, 8)])
+def test_p5_brute_force_exact_set(k, m, s, H):
+    rng = np.random.default_rng(11)
+    ins = "".join(rng.choice(list(BASES), 3000))
+    # queries: random text with a few inserted stretches spliced in
+    q = list("".join(rng.choice(list(BASES), 6000)))
+    for st in (100, 1700, 4000):
+        q[st:st + 200] = ins[st // 2:st // 2 + 200]
+    q = "".join(q)
+    members = {ins[i:i + k] for i in range(len(ins) - k + 1)}
+    o = oracle.OracleSBF(k, m, s, H, 1 << 13)          # small filter: false positives do occur
+    o.insert_records(ins)
+    bitmap, counts, nv = o.query_records(q)
+    bits = oracle.bitmap_bits(bitmap, len(q))
+    truth = np.array([q[i:i + k] in members for i in range(len(q) - k + 1)])
+    assert truth.sum() >= 3 * (200 - k + 1)
+    assert bits[:len(truth)][truth].all()              # no false negatives
+    assert not bits[len(truth):].any()
+    fp = np.count_nonzero(bits[:len(truth)] & ~truth)
+    assert counts[0] == truth.sum() + fp
+    # independent re-evaluation of every answer from exported bits with big-int arithmetic
+    words = o.words()
+    for p in range(0, len(truth), 7):
+        v = pack_str(q[p:p + k])
+        key = min(oracle.g(m, (v >> (2 * (k - m - i))) & ((1 << (2 * m)) - 1)) for i in range(k - m + 1))
+        shard = oracle.sigma(key, int(math.log2(o.num_shards)))
+        ok = True
+        for j in range(k - s + 1):
+            h = oracle.f(s, (v >> (2 * (k - s - j))) & ((1 << (2 * s)) - 1))
+            for i in range(H):
+                ok &= bool((int(words[shard, i % 4]) >> oracle.bitpos(h, i, H)) & 1)
+        assert ok == bits[p], p
+
+
+# ---------------------------------------------------------------- P6: order independence, idempotence, MT == ST
+def test_p6_order_independence_and_threads():
+    k = 31
+    seq = seqgen.markov(9, 3, 0.5, 200_000).copy()
+    seq[777:800] = ord("N")
+    cuts = np.sort(np.random.default_rng(3).choice(np.arange(1, seq.size), 40, replace=False))
+    offsets = np.concatenate(([0], cuts, [seq.size])).astype(np.uint64)
+    a = oracle.OracleSBF(k, 16, 28, 4, 1 << 21)
+    na = a.insert_records(seq, offsets)
+    ref = a.export_bits()
+    # permuted record order
+    perm = np.random.default_rng(4).permutation(len(offsets) - 1)
+    pieces = [seq[int(offsets[r]):int(offsets[r + 1])] for r in perm]
+    pseq = np.concatenate(pieces)
+    poff = np.concatenate(([0], np.cumsum([p.size for p in pieces]))).astype(np.uint64)
+    b = oracle.OracleSBF(k, 16, 28, 4, 1 << 21)
+    nb = b.insert_records(pseq, poff)
+    assert na == nb and (b.export_bits() == ref).all()
+    b.insert_records(pseq, poff)                       # inserting twice changes nothing
+    assert (b.export_bits() == ref).all()
+    # multi-core driver gives the same bits, bitmap and counts
+    c = oracle.OracleSBF(k, 16, 28, 4, 1 << 21)
+    assert c.insert_records(seq, offsets, threads=True) == na
+    assert (c.export_bits() == ref).all()
+    alien = seqgen.uniform(10, 150_000)
+    aoff = seqgen.fixed_offsets(1000, 150)
+    bm1, c1, n1 = a.query_records(alien, aoff)
+    bm2, c2, n2 = a.query_records(alien, aoff, threads=True)
+    assert n1 == n2 == 1000 * 120 and (bm1 == bm2).all() and (c1 == c2).all()
+
+
+# ---------------------------------------------------------------- P7: shard isolation
+@pytest.mark.parametrize("H", [1, 2, 4, 6, 8])
+def test_p7_shard_isolation(H):
+    k, m, s = 31, 16, 28
+    rng = np.random.default_rng(H)
+    o = oracle.OracleSBF(k, m, s, H, 1 << 20)
+    for _ in range(50):
+        o.clear()
+        kmer = "".join(rng.choice(list(BASES), k))
+        v = pack_str(kmer)
+        o.insert_kmer(v)
+        w = o.words()
+        nz = np.flatnonzero(w.any(axis=1))
+        assert nz.tolist() == [o.shard_of(v)]                         # only its own shard's 32 bytes
+        shard = int(nz[0])
+        nbits = sum(bin(int(x)).count("1") for x in w[shard])
+        assert 1 <= nbits <= H * (k - s + 1)                          # H*(k-s+1) bit positions
+        used = {i % 4 for i in range(H)}
+        for q in range(4):                                            # hash i -> sector word i mod 4
+            assert (int(w[shard, q]) != 0) == (q in used)
+        assert o.contains_kmer(v)
+
+
+# ---------------------------------------------------------------- P8: FPR band
+def _fill_prediction(o, z1):
+    """mean over shards of prod_{i<H} fill(word i mod 4)^(k-s+1): alien k-mers land uniformly on shards."""
+    w = o.words()
+    pc = np.zeros(w.shape, dtype=np.float64)
+    x = w.copy()
+    for _ in range(64):
+        pc += (x & np.uint64(1)).astype(np.float64)
+        x >>= np.uint64(1)
+    fill = pc / 64.0
+    per = np.ones(w.shape[0])
+    for i in range(o.H):
+        per *= fill[:, i % 4]
+    return float((per ** z1).mean())
+
+
+@pytest.mark.parametrize("m,s,H,log2bits", [(16, 28, 4, 20), (16, 28, 4, 22), (16, 31, 4, 22), (12, 24, 2, 22),
+                                            (20, 28, 8, 22), (16, 28, 1, 21), (16, 26, 6, 22)])
+def test_p8_fpr_matches_shard_fill(m, s, H, log2bits):
+    k = 31
+    seq = seqgen.uniform(1, 1_000_000)
+    alien = seqgen.uniform(2, 1_000_000)
+    o = oracle.OracleSBF(k, m, s, H, 1 << log2bits)
+    o.insert_records(seq, threads=True)
+    bitmap, counts, nv = o.query_records(alien, threads=True)
+    fpr = counts[0] / nv
+    pred = _fill_prediction(o, k - s + 1)
+    sigma3 = 3 * math.sqrt(max(pred * (1 - pred), 1e-12) / (nv / 8.5))     # positives are correlated inside runs
+    assert abs(fpr - pred) <= 0.05 * pred + sigma3, (fpr, pred)
+
+
+def test_p8_config1_fpr_saturated_and_relieved():
+    # BASELINE config 1: 2^20 bits for ~1e6 k-mers is saturated; at 2^24 bits the FPR must collapse
+    seq, alien = seqgen.uniform(1, 1_000_000), seqgen.uniform(2, 1_000_000)
+    fprs = []
+    for lb in (20, 24):
+        o = oracle.OracleSBF(31, 16, 28, 4, 1 << lb)
+        o.insert_records(seq, threads=True)
+        _, c, nv = o.query_records(alien, threads=True)
+        fprs.append(c[0] / nv)
+    assert 0.5 < fprs[0] < 0.99 and fprs[1] < 2e-3
+
+
+def test_p8_closed_form_per_shard_load():
+    """Eq.(1) per 64-bit sector word with the shard's own distinct s-mer count, then Eq.(2)."""
+    k, m, s, H = 31, 16, 28, 4
+    seq = seqgen.uniform(1, 300_000)
+    alien = seqgen.uniform(2, 1_000_000)
+    o = oracle.OracleSBF(k, m, s, H, 1 << 19)
+    o.insert_records(seq)
+    _, sh, valid = o.trace(seq)
+    n = seq.size - k + 1
+    S = bytes(seq)
+    # distinct (shard, s-mer) pairs: s-mer j..j+k-s of k-mer p go to shard(p)
+    pairs = set()
+    for p in range(n):
+        sp = int(sh[p])
+        for j in range(k - s + 1):
+            pairs.add((sp, S[p + j:p + j + s]))
+    n_j = np.bincount(np.fromiter((a for a, _ in pairs), dtype=np.int64), minlength=o.num_shards)
+    c = H / 4.0                                         # hashes per sector word
+    fill = 1 - (63 / 64) ** (c * n_j)
+    pred = float((fill ** (H * (k - s + 1))).mean())
+    _, counts, nv = o.query_records(alien, threads=True)
+    fpr = counts[0] / nv
+    assert -0.07 < fpr / pred - 1 < 0.25, (fpr, pred)
+
+
+# ---------------------------------------------------------------- P9: textbook special cases
+def test_p9_m_eq_k_s_eq_k_is_blocked_bloom():
+    """m = k = s: w = 1, one s-mer per k-mer -> a blocked Bloom filter over k-mers.
+    FPR = sum_j Poisson(j; n/B) * prod_words (1 - (63/64)^(c j))."""
+    k = m = s = 31
+    H = 4
+    seq = seqgen.uniform(1, 200_000)
+    alien = seqgen.uniform(2, 1_500_000)
+    o = oracle.OracleSBF(k, m, s, H, 1 << 20)          # 4096 blocks
+    n = o.insert_records(seq)
+    # exactly one shard and <= H bits per k-mer
+    lam = n / o.num_shards
+    j = np.arange(0, int(lam * 4) + 50)
+    logp = j * math.log(lam) - lam - np.array([math.lgamma(x + 1) for x in j])
+    pois = np.exp(logp)
+    pred = float((pois * (1 - (63 / 64) ** j) ** H).sum())
+    _, counts, nv = o.query_records(alien, threads=True)
+    fpr = counts[0] / nv
+    assert abs(fpr / pred - 1) < 0.05, (fpr, pred)
+    # and the shard of a k-mer is sigma(g(k-mer)) when w = 1
+    v = o.pack_kmer(seq, 1234)
+    assert o.shard_of(v) == oracle.sigma(oracle.g(k, v), 12)
+
+
+def test_p9_findere_overlap_lowers_fpr():
+    """Eq.(2): at equal memory, more overlapping s-mers suppress alien false positives (s=28 < s=30 < s=31)."""
+    seq, alien = seqgen.uniform(1, 1_000_000), seqgen.uniform(2, 1_000_000)
+    fpr = {}
+    for s in (28, 30, 31):
+        o = oracle.OracleSBF(31, 16, s, 4, 1 << 23)
+        o.insert_records(seq, threads=True)
+        _, c, nv = o.query_records(alien, threads=True)
+        fpr[s] = c[0] / nv
+    assert fpr[28] < fpr[30] < fpr[31], fpr
+
+
+def test_create_rejects_bad_parameters():
+    for args in [(0, 1, 1, 1, 256), (33, 16, 28, 4, 256), (31, 32, 28, 4, 256), (31, 16, 32, 4, 256),
+                 (31, 16, 28, 0, 256), (31, 16, 28, 4, 0), (31, 0, 28, 4, 256), (31, 16, 0, 4, 256)]:
+        with pytest.raises(ValueError):
+            oracle.OracleSBF(*args)
+    # A8: shard count = next power of two >= ceil(num_bits / 256)
+    for bits, shards in [(1, 1), (256, 1), (257, 2), (1 << 20, 4096), ((1 << 20) + 1, 8192), (3 * 256, 4)]:
+        assert oracle.OracleSBF(31, 16, 28, 4, bits).num_shards == shards
