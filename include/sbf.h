@@ -1,0 +1,154 @@
+/*
+ * sbf.h — C ABI of the B200-native Super Bloom filter insert/query hot path.
+ *
+ * What the library computes is defined by the paper (arxiv 2606.24417, "cuSBF";
+ * P:<n> = line n of its extracted text PAPER.md) and, where the paper gives no
+ * constants or edge rules, by the readings A1-A18 in DESIGN.md §3:
+ *
+ *   a k-mer v (2 bits/base, first base most significant) is mapped to
+ *     minKey = min over its k-m+1 m-mers of g(m-mer)             (A1)
+ *     shard  = sigma(minKey) in [0, 2^P)                         (A2)
+ *     for each of its k-s+1 s-mers x, h = f(x), and for i < H the bit
+ *     B(h,i) of 64-bit sector word (i mod 4) of that shard       (A4, A5)
+ *   insert sets those H*(k-s+1) bits (Alg. 1); query reports the k-mer
+ *   present iff every one of them is set — the Findere rule (Alg. 2).
+ *   A k-mer containing a non-ACGT symbol or running past the end of its record
+ *   does not exist: it is never inserted and queries false.
+ *
+ * Conventions
+ *   - All `d_*` pointers are DEVICE pointers owned by the caller; all `h_*`
+ *     pointers are HOST pointers owned by the caller.  The library owns the
+ *     filter and its scratch buffers (on the device that was current at
+ *     sbf_create()).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
+ *     stream).  Device-facing calls only enqueue work on `stream` and never
+ *     synchronise; exception: when the internal scratch must grow,
+ *     the call performs a cudaMalloc (implicitly synchronising).  Call
+ *     sbf_reserve() up front to avoid that.  One call in flight per handle.
+ *   - Every function returns SBF_OK (0) or a negative sbf_status; nothing
+ *     throws across this boundary.  sbf_last_error() gives a message for the
+ *     last failure on the calling thread.
+ *   - There is no CPU fallback: without a CUDA device sbf_create() fails.
+ */
+#ifndef SBF_H
+#define SBF_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sbf sbf_t; /* opaque */
+
+typedef enum sbf_status {
+    SBF_OK = 0,
+    SBF_ERR_INVALID_ARG = -1, /* NULL handle/pointer, bad sizes */
+    SBF_ERR_UNSUPPORTED = -2, /* parameter combination outside what the kernels support */
+    SBF_ERR_NOMEM = -3,       /* device or host allocation failed */
+    SBF_ERR_CUDA = -4         /* any other CUDA runtime error (message in sbf_last_error) */
+} sbf_status;
+
+/*
+ * sbf_create — allocate a zeroed filter (A8).
+ *   1 <= k <= 32 (one 64-bit word per packed k-mer); 1 <= m <= k; 1 <= s <= k;
+ *   1 <= H <= 32 (H <= 10 uses bit-slicing A5, H > 10 the salted multiply A6);
+ *   num_bits >= 1.  numShards = next power of two >= ceil(num_bits/256), at most 2^32.
+ *   Layout in device memory (A12): shard-major, four little-endian 64-bit sector words
+ *   per shard, 32 bytes per shard, 32-byte aligned (one L2 sector per shard).
+ *   (k,m,s,H) combinations compiled as specialised streaming kernels run those; every
+ *   other legal combination runs a runtime-parameter CUDA kernel (same bits, slower).
+ *   Returns NULL on error.
+ */
+sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits);
+
+/* sbf_destroy — free filter and scratch.  Synchronises the device.  NULL is ignored. */
+void sbf_destroy(sbf_t *f);
+
+/* Geometry of the filter actually allocated (A8): 256 * numShards bits. */
+uint64_t sbf_num_bits(const sbf_t *f);
+uint64_t sbf_num_shards(const sbf_t *f);
+/* 1 if (k,m,s,H) runs the specialised streaming kernels, 0 if it runs the runtime-parameter kernels. */
+int sbf_is_specialized(const sbf_t *f);
+
+/* sbf_reserve — pre-size the internal scratch (2-bit packed sequence + validity mask)
+ * for batches of up to max_bases symbols, so later calls never allocate. */
+int sbf_reserve(sbf_t *f, uint64_t max_bases);
+
+/* sbf_clear — zero the filter, stream-ordered. */
+int sbf_clear(sbf_t *f, void *stream);
+
+/*
+ * sbf_insert_seq — insert every valid k-mer of one sequence (Alg. 1).
+ *   d_seq: `len` ASCII symbols on the device.  A,C,G,T in either case are valid (A9);
+ *   any other byte is invalid and k-mers covering it are skipped.  len may be 0.
+ */
+int sbf_insert_seq(sbf_t *f, const char *d_seq, uint64_t len, void *stream);
+
+/*
+ * sbf_insert_records — insert a dense batch of records ("dense record batch").
+ *   d_bases: the records' symbols concatenated, `total_bases` bytes, no separators.
+ *   d_offsets: n_rec+1 non-decreasing device uint64, d_offsets[0] = 0,
+ *   d_offsets[n_rec] = total_bases; record r = d_bases[d_offsets[r] .. d_offsets[r+1]).
+ *   Empty records are allowed.  No k-mer spans two records.
+ *   total_bases is passed by value so the call needs no device->host read.
+ */
+int sbf_insert_records(sbf_t *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec,
+                       uint64_t total_bases, void *stream);
+
+/*
+ * sbf_query_seq — query every k-mer start position of one sequence (Alg. 2).
+ *   d_bitmap: ceil(len/32) device uint32 words, all written (no pre-zeroing needed):
+ *   bit p (word p>>5, bit p&31) = 1 iff a valid k-mer starts at symbol p and all its
+ *   H*(k-s+1) bits are set; invalid k-mers and the last k-1 positions give 0 (A11).
+ *   d_hits: NULL, or one device uint64 that receives the number of set bits.
+ */
+int sbf_query_seq(sbf_t *f, const char *d_seq, uint64_t len, uint32_t *d_bitmap, uint64_t *d_hits,
+                  void *stream);
+
+/*
+ * sbf_query_records — same for a dense record batch; bit index = position in the
+ *   concatenated buffer; d_bitmap has ceil(total_bases/32) words.
+ *   d_hit_counts: NULL, or n_rec device uint32: set bits of record r.
+ */
+int sbf_query_records(sbf_t *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec,
+                      uint64_t total_bases, uint32_t *d_bitmap, uint32_t *d_hit_counts, void *stream);
+
+/*
+ * Host-facing forms ("host-facing calls synchronise").  The symbols (and offsets,
+ * and results) live in HOST memory; the library stages them through pinned buffers in
+ * chunks, overlapping the copies with the kernels on two internal streams,
+ * and returns after everything has completed.  h_bitmap / h_hit_counts as above, on the host.
+ */
+int sbf_insert_seq_host(sbf_t *f, const char *h_seq, uint64_t len);
+int sbf_insert_records_host(sbf_t *f, const char *h_bases, const uint64_t *h_offsets, uint64_t n_rec);
+int sbf_query_seq_host(sbf_t *f, const char *h_seq, uint64_t len, uint32_t *h_bitmap, uint64_t *h_hits);
+int sbf_query_records_host(sbf_t *f, const char *h_bases, const uint64_t *h_offsets, uint64_t n_rec,
+                           uint32_t *h_bitmap, uint32_t *h_hit_counts);
+
+/* sbf_export_bits — copy the filter (32*numShards bytes, layout A12) to host memory.
+ * nbytes must equal 32*numShards.  Synchronises the device. */
+int sbf_export_bits(const sbf_t *f, void *h_dst, uint64_t nbytes);
+/* sbf_import_bits — the inverse: overwrite the filter from host memory.  Synchronises. */
+int sbf_import_bits(sbf_t *f, const void *h_src, uint64_t nbytes);
+/* sbf_filter_device_ptr — the filter's device address (read-only use by the caller, e.g. a
+ * multi-GPU OR-reduce of replicas). */
+const uint64_t *sbf_filter_device_ptr(const sbf_t *f);
+/* sbf_or_bits_device — filter |= d_src (32*numShards bytes on the device), stream-ordered.
+ * The merge step of the replica scheme. */
+int sbf_or_bits_device(sbf_t *f, const uint64_t *d_src, uint64_t nbytes, void *stream);
+
+/* Message for the last error on the calling thread ("" if none). */
+const char *sbf_last_error(void);
+
+/* Counts kernels launched by this library in this process (all handles); bench.py reports it. */
+uint64_t sbf_kernel_launches(void);
+
+/* Diagnostics for tests: dump the internal 2-bit packed words / validity mask of the LAST batch
+ * (device->host, synchronises).  n_words = ceil(bases/16); mask has one uint16 per word. */
+int sbf_debug_last_packed(const sbf_t *f, uint32_t *h_words, uint16_t *h_mask, uint64_t n_words);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SBF_H */

@@ -1,0 +1,618 @@
+// sbf_api.cu — the C ABI of include/sbf.h: handle, scratch, kernel dispatch, host-facing staging.
+// Every step of the path (pack, minimizer, shard, s-mer hashing, merge, result bitmap, hit counts)
+// runs in the kernels of sbf_device.cuh; this file only sizes buffers and enqueues launches.
+#include "../../include/sbf.h"
+
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#define SBF_DEFINE_AUX_KERNELS
+#include "sbf_dispatch.h"
+
+using namespace sbfk;
+
+namespace {
+
+thread_local std::string g_err;
+std::atomic<uint64_t> g_launches{0};
+
+int fail(int code, const char *what)
+{
+    g_err = what;
+    return code;
+}
+int fail_cuda(cudaError_t e, const char *where)
+{
+    g_err = std::string(where) + ": " + cudaGetErrorString(e);
+    return e == cudaErrorMemoryAllocation ? SBF_ERR_NOMEM : SBF_ERR_CUDA;
+}
+#define CK(call)                                                  \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return fail_cuda(e__, #call);     \
+    } while (0)
+
+const KernelEntry *find_entry(int k, int m, int s, int H)
+{
+    typedef const KernelEntry *(*table_fn)(int *);
+    static const table_fn tables[] = {inst_table_default, inst_table_s_axis, inst_table_m_axis, inst_table_h_axis,
+                                      inst_table_small};
+    for (table_fn t : tables) {
+        int n = 0;
+        const KernelEntry *e = t(&n);
+        for (int i = 0; i < n; ++i)
+            if (e[i].k == k && e[i].m == m && e[i].s == s && e[i].H == H) return &e[i];
+    }
+    return nullptr;
+}
+
+struct HostRun { // persistent state of the host-facing path (two slots: copy c+1 while computing c)
+    cudaStream_t copy = nullptr, comp = nullptr;
+    cudaEvent_t copied[2] = {nullptr, nullptr}, computed[2] = {nullptr, nullptr};
+    char *pin[2] = {nullptr, nullptr};     // pinned staging for symbols (pageable caller memory only)
+    char *d_bases[2] = {nullptr, nullptr};
+    uint64_t *h_off[2] = {nullptr, nullptr};
+    uint64_t *d_off[2] = {nullptr, nullptr};
+    uint64_t cap_pin = 0, cap_bases = 0, cap_off = 0;
+    uint32_t *d_bitmap = nullptr;  uint64_t cap_bitmap = 0;
+    uint64_t *d_off_full = nullptr; uint32_t *d_counts = nullptr; uint64_t cap_rec = 0;
+    unsigned long long *d_hits = nullptr;
+    ~HostRun()
+    {
+        for (int i = 0; i < 2; ++i) {
+            if (copied[i]) cudaEventDestroy(copied[i]);
+            if (computed[i]) cudaEventDestroy(computed[i]);
+            if (pin[i]) cudaFreeHost(pin[i]);
+            if (h_off[i]) cudaFreeHost(h_off[i]);
+            if (d_bases[i]) cudaFree(d_bases[i]);
+            if (d_off[i]) cudaFree(d_off[i]);
+        }
+        if (d_bitmap) cudaFree(d_bitmap);
+        if (d_off_full) cudaFree(d_off_full);
+        if (d_counts) cudaFree(d_counts);
+        if (d_hits) cudaFree(d_hits);
+        if (copy) cudaStreamDestroy(copy);
+        if (comp) cudaStreamDestroy(comp);
+        cudaGetLastError();
+    }
+};
+
+} // namespace
+
+struct sbf {
+    int k, m, s, H, P;
+    int device;
+    uint64_t num_shards;
+    uint64_t *filter;        // 4 * num_shards words
+    const KernelEntry *entry; // nullptr -> runtime-parameter kernels
+    // scratch of the last batch
+    uint32_t *packed;
+    uint16_t *gmask;
+    uint64_t cap_words;       // allocated words in packed / gmask
+    uint64_t last_words;      // words written by the last pack
+    // L2 persistence window (a7)
+    bool l2_window;
+    cudaStream_t l2_stream_set;
+    bool l2_stream_valid;
+    // host-facing staging (created on first use)
+    HostRun *host;
+};
+
+namespace {
+
+uint64_t words_for(uint64_t n_bases) { return (n_bases + 15) / 16 + kPadWords; }
+
+int ensure_scratch(sbf *f, uint64_t n_bases)
+{
+    uint64_t need = words_for(n_bases);
+    if (need <= f->cap_words) return SBF_OK;
+    if (f->packed) cudaFree(f->packed);
+    if (f->gmask) cudaFree(f->gmask);
+    f->packed = nullptr; f->gmask = nullptr; f->cap_words = 0;
+    uint64_t cap = need + need / 8;
+    CK(cudaMalloc(&f->packed, cap * sizeof(uint32_t)));
+    CK(cudaMalloc(&f->gmask, cap * sizeof(uint16_t) + 8));
+    f->cap_words = cap;
+    return SBF_OK;
+}
+
+// a7: keep a filter that fits in L2 resident there (accessPolicyWindow on the caller's stream)
+void apply_l2_window(sbf *f, cudaStream_t st)
+{
+    if (!f->l2_window) return;
+    if (f->l2_stream_valid && f->l2_stream_set == st) return;
+    cudaStreamAttrValue v;
+    memset(&v, 0, sizeof(v));
+    v.accessPolicyWindow.base_ptr = f->filter;
+    v.accessPolicyWindow.num_bytes = f->num_shards * 32;
+    v.accessPolicyWindow.hitRatio = 1.0f;
+    v.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+    v.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+    if (cudaStreamSetAttribute(st, cudaStreamAttributeAccessPolicyWindow, &v) != cudaSuccess) {
+        cudaGetLastError();
+        f->l2_window = false;
+        return;
+    }
+    f->l2_stream_set = st;
+    f->l2_stream_valid = true;
+}
+
+// a1: pack + validity mask (+ record ends) of one batch into the scratch
+int run_pack(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, cudaStream_t st)
+{
+    int rc = ensure_scratch(f, total);
+    if (rc) return rc;
+    uint64_t nw = words_for(total);
+    f->last_words = nw;
+    unsigned blocks = (unsigned)((nw + 255) / 256);
+    int aligned = ((reinterpret_cast<uintptr_t>(d_bases) & 15) == 0) ? 1 : 0;
+    pack_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<const uint8_t *>(d_bases), total, f->packed, f->gmask, nw, f->k,
+                                        aligned);
+    CK(cudaGetLastError());
+    g_launches++;
+    if (d_offsets && n_rec > 0 && f->k >= 2 && total > 0) {
+        unsigned b2 = (unsigned)((n_rec + 255) / 256);
+        mark_ends_kernel<<<b2, 256, 0, st>>>(d_offsets, n_rec, total, reinterpret_cast<uint32_t *>(f->gmask));
+        CK(cudaGetLastError());
+        g_launches++;
+    }
+    return SBF_OK;
+}
+
+StreamParams make_params(sbf *f, uint64_t total, uint32_t *bitmap)
+{
+    StreamParams p;
+    p.packed = f->packed;
+    p.gmask = f->gmask;
+    p.n_pos = total;
+    p.filter = f->filter;
+    p.shard_shift = 32 - f->P;
+    p.bitmap = bitmap;
+    p.n_bitmap_words = (total + 31) / 32;
+    return p;
+}
+
+template <bool INSERT>
+int run_main(sbf *f, uint64_t total, uint32_t *bitmap, cudaStream_t st)
+{
+    if (total == 0) return SBF_OK;
+    StreamParams p = make_params(f, total, bitmap);
+    if (f->entry) {
+        CK((INSERT ? f->entry->insert : f->entry->query)(p, st));
+    } else {
+        NaiveParams np;
+        np.sp = p; np.k = f->k; np.m = f->m; np.s = f->s; np.H = f->H;
+        uint64_t n32 = (total + 31) / 32 * 32;
+        unsigned blocks = (unsigned)((n32 + 255) / 256);
+        naive_kernel<INSERT><<<blocks, 256, 0, st>>>(np);
+        CK(cudaGetLastError());
+    }
+    g_launches++;
+    return SBF_OK;
+}
+
+int run_insert(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, cudaStream_t st)
+{
+    if (total == 0) return SBF_OK;
+    apply_l2_window(f, st);
+    int rc = run_pack(f, d_bases, d_offsets, n_rec, total, st);
+    if (rc) return rc;
+    return run_main<true>(f, total, nullptr, st);
+}
+
+int run_query(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, uint32_t *d_bitmap,
+              cudaStream_t st)
+{
+    if (total == 0) return SBF_OK;
+    apply_l2_window(f, st);
+    int rc = run_pack(f, d_bases, d_offsets, n_rec, total, st);
+    if (rc) return rc;
+    return run_main<false>(f, total, d_bitmap, st);
+}
+
+int run_count_records(const uint32_t *d_bitmap, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, uint32_t *d_counts,
+                      cudaStream_t st)
+{
+    if (n_rec == 0) return SBF_OK;
+    if (total / n_rec < 2048) {
+        unsigned blocks = (unsigned)((n_rec + 255) / 256);
+        count_records_thread_kernel<<<blocks, 256, 0, st>>>(d_bitmap, d_offsets, n_rec, d_counts);
+    } else {
+        unsigned blocks = (unsigned)(n_rec < 4096 ? n_rec : 4096);
+        count_records_block_kernel<<<blocks, 256, 0, st>>>(d_bitmap, d_offsets, n_rec, d_counts);
+    }
+    CK(cudaGetLastError());
+    g_launches++;
+    return SBF_OK;
+}
+
+} // namespace
+
+// =============================================================================================
+// C ABI — device-facing
+// =============================================================================================
+extern "C" {
+
+const char *sbf_last_error(void) { return g_err.c_str(); }
+uint64_t sbf_kernel_launches(void) { return g_launches.load(); }
+
+sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits)
+{
+    g_err.clear();
+    if (k < 1 || k > 32 || m < 1 || m > k || s < 1 || s > k || H < 1 || H > 32 || num_bits < 1) {
+        fail(SBF_ERR_INVALID_ARG, "sbf_create: need 1<=k<=32, 1<=m<=k, 1<=s<=k, 1<=H<=32, num_bits>=1");
+        return nullptr;
+    }
+    uint64_t need = (num_bits + 255) / 256, shards = 1;
+    int P = 0;
+    while (shards < need) { shards <<= 1; ++P; } // rounded up to a power of two (A8)
+    if (P > 32) {
+        fail(SBF_ERR_UNSUPPORTED, "sbf_create: more than 2^32 shards");
+        return nullptr;
+    }
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) {
+        fail_cuda(e, "sbf_create: no CUDA device (this library has no CPU fallback)");
+        return nullptr;
+    }
+    sbf *f = new (std::nothrow) sbf();
+    if (!f) {
+        fail(SBF_ERR_NOMEM, "sbf_create: host allocation failed");
+        return nullptr;
+    }
+    f->k = k; f->m = m; f->s = s; f->H = H; f->P = P; f->device = dev;
+    f->num_shards = shards;
+    f->entry = find_entry(k, m, s, H);
+    e = cudaMalloc(&f->filter, shards * 32);
+    if (e == cudaSuccess) e = cudaMemset(f->filter, 0, shards * 32);
+    if (e != cudaSuccess) {
+        fail_cuda(e, "sbf_create: filter allocation");
+        if (f->filter) cudaFree(f->filter);
+        delete f;
+        return nullptr;
+    }
+    // a7: L2 persistence window when the whole filter fits the persisting carve-out
+    int max_persist = 0, max_window = 0;
+    cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev);
+    cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev);
+    uint64_t bytes = shards * 32;
+    if (max_persist > 0 && bytes <= (uint64_t)max_persist && bytes <= (uint64_t)max_window && bytes >= (1u << 20)) {
+        size_t cur = 0;
+        cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize);
+        if (cur < bytes) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)max_persist);
+        f->l2_window = (cudaGetLastError() == cudaSuccess);
+    }
+    return f;
+}
+
+void sbf_destroy(sbf_t *f)
+{
+    if (!f) return;
+    cudaDeviceSynchronize();
+    delete f->host;
+    if (f->packed) cudaFree(f->packed);
+    if (f->gmask) cudaFree(f->gmask);
+    if (f->filter) cudaFree(f->filter);
+    cudaGetLastError();
+    delete f;
+}
+
+uint64_t sbf_num_bits(const sbf_t *f) { return f ? f->num_shards * 256 : 0; }
+uint64_t sbf_num_shards(const sbf_t *f) { return f ? f->num_shards : 0; }
+int sbf_is_specialized(const sbf_t *f) { return (f && f->entry) ? 1 : 0; }
+const uint64_t *sbf_filter_device_ptr(const sbf_t *f) { return f ? f->filter : nullptr; }
+
+int sbf_reserve(sbf_t *f, uint64_t max_bases)
+{
+    if (!f) return fail(SBF_ERR_INVALID_ARG, "sbf_reserve: NULL handle");
+    return ensure_scratch(f, max_bases);
+}
+
+int sbf_clear(sbf_t *f, void *stream)
+{
+    if (!f) return fail(SBF_ERR_INVALID_ARG, "sbf_clear: NULL handle");
+    CK(cudaMemsetAsync(f->filter, 0, f->num_shards * 32, (cudaStream_t)stream));
+    return SBF_OK;
+}
+
+int sbf_insert_seq(sbf_t *f, const char *d_seq, uint64_t len, void *stream)
+{
+    if (!f || (!d_seq && len)) return fail(SBF_ERR_INVALID_ARG, "sbf_insert_seq: NULL argument");
+    return run_insert(f, d_seq, nullptr, 0, len, (cudaStream_t)stream);
+}
+
+int sbf_insert_records(sbf_t *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total_bases,
+                       void *stream)
+{
+    if (!f || (!d_bases && total_bases) || (!d_offsets && n_rec)) return fail(SBF_ERR_INVALID_ARG, "sbf_insert_records: NULL argument");
+    if (n_rec == 0 && total_bases) return fail(SBF_ERR_INVALID_ARG, "sbf_insert_records: bases without records");
+    return run_insert(f, d_bases, d_offsets, n_rec, total_bases, (cudaStream_t)stream);
+}
+
+int sbf_query_seq(sbf_t *f, const char *d_seq, uint64_t len, uint32_t *d_bitmap, uint64_t *d_hits, void *stream)
+{
+    if (!f || (!d_seq && len) || (!d_bitmap && len)) return fail(SBF_ERR_INVALID_ARG, "sbf_query_seq: NULL argument");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = run_query(f, d_seq, nullptr, 0, len, d_bitmap, st);
+    if (rc) return rc;
+    if (d_hits) {
+        CK(cudaMemsetAsync(d_hits, 0, sizeof(uint64_t), st));
+        uint64_t nw = (len + 31) / 32;
+        if (nw) {
+            unsigned blocks = (unsigned)((nw + 255) / 256 < 1184 ? (nw + 255) / 256 : 1184);
+            count_total_kernel<<<blocks, 256, 0, st>>>(d_bitmap, nw, reinterpret_cast<unsigned long long *>(d_hits));
+            CK(cudaGetLastError());
+            g_launches++;
+        }
+    }
+    return SBF_OK;
+}
+
+int sbf_query_records(sbf_t *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total_bases,
+                      uint32_t *d_bitmap, uint32_t *d_hit_counts, void *stream)
+{
+    if (!f || (!d_bases && total_bases) || (!d_offsets && n_rec) || (!d_bitmap && total_bases))
+        return fail(SBF_ERR_INVALID_ARG, "sbf_query_records: NULL argument");
+    if (n_rec == 0 && total_bases) return fail(SBF_ERR_INVALID_ARG, "sbf_query_records: bases without records");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = run_query(f, d_bases, d_offsets, n_rec, total_bases, d_bitmap, st);
+    if (rc) return rc;
+    if (d_hit_counts && n_rec) {
+        if (total_bases == 0) {
+            CK(cudaMemsetAsync(d_hit_counts, 0, n_rec * sizeof(uint32_t), st));
+        } else {
+            rc = run_count_records(d_bitmap, d_offsets, n_rec, total_bases, d_hit_counts, st);
+            if (rc) return rc;
+        }
+    }
+    return SBF_OK;
+}
+
+int sbf_export_bits(const sbf_t *f, void *h_dst, uint64_t nbytes)
+{
+    if (!f || !h_dst) return fail(SBF_ERR_INVALID_ARG, "sbf_export_bits: NULL argument");
+    if (nbytes != f->num_shards * 32) return fail(SBF_ERR_INVALID_ARG, "sbf_export_bits: nbytes must be 32*numShards");
+    CK(cudaDeviceSynchronize());
+    CK(cudaMemcpy(h_dst, f->filter, nbytes, cudaMemcpyDeviceToHost));
+    return SBF_OK;
+}
+
+int sbf_import_bits(sbf_t *f, const void *h_src, uint64_t nbytes)
+{
+    if (!f || !h_src) return fail(SBF_ERR_INVALID_ARG, "sbf_import_bits: NULL argument");
+    if (nbytes != f->num_shards * 32) return fail(SBF_ERR_INVALID_ARG, "sbf_import_bits: nbytes must be 32*numShards");
+    CK(cudaDeviceSynchronize());
+    CK(cudaMemcpy(f->filter, h_src, nbytes, cudaMemcpyHostToDevice));
+    return SBF_OK;
+}
+
+int sbf_or_bits_device(sbf_t *f, const uint64_t *d_src, uint64_t nbytes, void *stream)
+{
+    if (!f || !d_src) return fail(SBF_ERR_INVALID_ARG, "sbf_or_bits_device: NULL argument");
+    if (nbytes != f->num_shards * 32) return fail(SBF_ERR_INVALID_ARG, "sbf_or_bits_device: nbytes must be 32*numShards");
+    uint64_t nw = f->num_shards * 4;
+    unsigned blocks = (unsigned)((nw / 2 + 255) / 256 < 2368 ? (nw / 2 + 255) / 256 : 2368);
+    or_words_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(f->filter, d_src, nw);
+    CK(cudaGetLastError());
+    g_launches++;
+    return SBF_OK;
+}
+
+int sbf_debug_last_packed(const sbf_t *f, uint32_t *h_words, uint16_t *h_mask, uint64_t n_words)
+{
+    if (!f || !h_words || !h_mask) return fail(SBF_ERR_INVALID_ARG, "sbf_debug_last_packed: NULL argument");
+    if (n_words > f->last_words) return fail(SBF_ERR_INVALID_ARG, "sbf_debug_last_packed: more words than the last batch");
+    CK(cudaDeviceSynchronize());
+    CK(cudaMemcpy(h_words, f->packed, n_words * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(h_mask, f->gmask, n_words * sizeof(uint16_t), cudaMemcpyDeviceToHost));
+    return SBF_OK;
+}
+
+} // extern "C"
+
+// =============================================================================================
+// C ABI — host-facing ("host-facing calls synchronise"; staging after P:323-325):
+// the batch is cut in chunks of kHostChunk symbols that overlap by k-1, so that every k-mer
+// start position belongs to exactly one chunk and is complete inside it.  A copy stream moves
+// chunk c+1 to the device while the compute stream packs and walks chunk c; results come back
+// chunk by chunk.  Pageable caller memory is staged through two pinned buffers; pinned or
+// registered caller memory is copied from directly.
+// =============================================================================================
+namespace {
+
+constexpr uint64_t kHostChunk = 64ull << 20; // symbols per chunk, multiple of 128
+
+bool is_pinned(const void *p)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeHost;
+}
+
+// insert (h_bitmap == nullptr) or query of a host-resident batch
+int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets, uint64_t n_rec, uint64_t total,
+             uint32_t *h_bitmap, uint32_t *h_counts, uint64_t *h_hits)
+{
+    if (h_counts && n_rec) memset(h_counts, 0, n_rec * sizeof(uint32_t));
+    if (h_hits) *h_hits = 0;
+    if (total == 0) return SBF_OK;
+    const uint64_t ov = (uint64_t)f->k - 1;
+    const uint64_t span = (total < kHostChunk ? total : kHostChunk) + ov; // largest chunk incl. overlap
+    const uint64_t n_chunks = (total + kHostChunk - 1) / kHostChunk;
+    const bool direct = is_pinned(h_bases);
+    // most record boundaries a chunk can hold: all of them, bounded by its symbols (+2 ends)
+    uint64_t max_off = (n_rec + 2 < span + 2 ? n_rec + 2 : span + 2);
+    if (!h_offsets) max_off = 2;
+
+    if (!f->host) {
+        f->host = new (std::nothrow) HostRun();
+        if (!f->host) return fail(SBF_ERR_NOMEM, "host staging: allocation failed");
+        CK(cudaStreamCreateWithFlags(&f->host->copy, cudaStreamNonBlocking));
+        CK(cudaStreamCreateWithFlags(&f->host->comp, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CK(cudaEventCreateWithFlags(&f->host->copied[i], cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&f->host->computed[i], cudaEventDisableTiming));
+        }
+    }
+    HostRun &R = *f->host;
+    const int slots = n_chunks > 1 ? 2 : 1;
+    if (R.cap_bases < span) { // grow the device symbol slots (both, so a later multi-chunk call finds them)
+        for (int i = 0; i < 2; ++i) {
+            if (R.d_bases[i]) cudaFree(R.d_bases[i]);
+            R.d_bases[i] = nullptr;
+        }
+        R.cap_bases = 0;
+        for (int i = 0; i < 2; ++i) CK(cudaMalloc(&R.d_bases[i], span + 16));
+        R.cap_bases = span;
+    }
+    if (!direct && R.cap_pin < span) {
+        for (int i = 0; i < 2; ++i) {
+            if (R.pin[i]) cudaFreeHost(R.pin[i]);
+            R.pin[i] = nullptr;
+        }
+        R.cap_pin = 0;
+        for (int i = 0; i < 2; ++i) CK(cudaMallocHost(&R.pin[i], span));
+        R.cap_pin = span;
+    }
+    if (h_offsets && R.cap_off < max_off) {
+        for (int i = 0; i < 2; ++i) {
+            if (R.h_off[i]) cudaFreeHost(R.h_off[i]);
+            if (R.d_off[i]) cudaFree(R.d_off[i]);
+            R.h_off[i] = nullptr; R.d_off[i] = nullptr;
+        }
+        R.cap_off = 0;
+        for (int i = 0; i < 2; ++i) {
+            CK(cudaMallocHost(&R.h_off[i], max_off * sizeof(uint64_t)));
+            CK(cudaMalloc(&R.d_off[i], max_off * sizeof(uint64_t)));
+        }
+        R.cap_off = max_off;
+    }
+    (void)slots;
+    const uint64_t n_bm = (total + 31) / 32;
+    if (!insert) {
+        if (R.cap_bitmap < n_bm + 4) {
+            if (R.d_bitmap) cudaFree(R.d_bitmap);
+            R.d_bitmap = nullptr; R.cap_bitmap = 0;
+            CK(cudaMalloc(&R.d_bitmap, (n_bm + 4) * sizeof(uint32_t)));
+            R.cap_bitmap = n_bm + 4;
+        }
+        if (h_counts && n_rec) {
+            if (R.cap_rec < n_rec) {
+                if (R.d_off_full) cudaFree(R.d_off_full);
+                if (R.d_counts) cudaFree(R.d_counts);
+                R.d_off_full = nullptr; R.d_counts = nullptr; R.cap_rec = 0;
+                CK(cudaMalloc(&R.d_off_full, (n_rec + 1) * sizeof(uint64_t)));
+                CK(cudaMalloc(&R.d_counts, n_rec * sizeof(uint32_t)));
+                R.cap_rec = n_rec;
+            }
+            CK(cudaMemcpyAsync(R.d_off_full, h_offsets, (n_rec + 1) * sizeof(uint64_t), cudaMemcpyHostToDevice, R.copy));
+        }
+        if (h_hits && !R.d_hits) CK(cudaMalloc(&R.d_hits, sizeof(unsigned long long)));
+    }
+    int rc = ensure_scratch(f, span);
+    if (rc) return rc;
+
+    uint64_t off_lo = 0; // first offset index with h_offsets[i] > chunk start (monotone over chunks)
+    for (uint64_t c = 0; c < n_chunks; ++c) {
+        const int sl = (int)(c & 1);
+        const uint64_t a = c * kHostChunk;
+        const uint64_t e = (a + kHostChunk + ov < total) ? a + kHostChunk + ov : total;
+        const uint64_t n = e - a;
+        if (c >= 2) {
+            CK(cudaEventSynchronize(R.copied[sl]));                 // pinned slot free again
+            CK(cudaStreamWaitEvent(R.copy, R.computed[sl], 0));     // device slot free again
+        }
+        uint64_t n_off = 0;
+        if (h_offsets) {
+            while (off_lo <= n_rec && h_offsets[off_lo] <= a) ++off_lo;
+            uint64_t *ho = R.h_off[sl];
+            ho[n_off++] = 0;
+            for (uint64_t i = off_lo; i <= n_rec && h_offsets[i] < e; ++i) ho[n_off++] = h_offsets[i] - a;
+            ho[n_off++] = n;
+            CK(cudaMemcpyAsync(R.d_off[sl], ho, n_off * sizeof(uint64_t), cudaMemcpyHostToDevice, R.copy));
+        }
+        const char *src = h_bases + a;
+        if (!direct) {
+            memcpy(R.pin[sl], src, n);
+            src = R.pin[sl];
+        }
+        CK(cudaMemcpyAsync(R.d_bases[sl], src, n, cudaMemcpyHostToDevice, R.copy));
+        CK(cudaEventRecord(R.copied[sl], R.copy));
+        CK(cudaStreamWaitEvent(R.comp, R.copied[sl], 0));
+        const uint64_t *d_off = h_offsets ? R.d_off[sl] : nullptr;
+        const uint64_t nr = h_offsets ? n_off - 1 : 0;
+        if (insert) {
+            rc = run_insert(f, R.d_bases[sl], d_off, nr, n, R.comp);
+        } else {
+            rc = run_query(f, R.d_bases[sl], d_off, nr, n, R.d_bitmap + a / 32, R.comp);
+        }
+        if (rc) return rc;
+        CK(cudaEventRecord(R.computed[sl], R.comp));
+        if (!insert && h_bitmap) {
+            const uint64_t w0 = a / 32;
+            const uint64_t w1 = (c + 1 == n_chunks) ? n_bm : (a + kHostChunk) / 32;
+            CK(cudaMemcpyAsync(h_bitmap + w0, R.d_bitmap + w0, (w1 - w0) * sizeof(uint32_t), cudaMemcpyDeviceToHost, R.comp));
+        }
+    }
+    if (!insert) {
+        CK(cudaStreamSynchronize(R.copy));
+        if (h_counts && n_rec) {
+            rc = run_count_records(R.d_bitmap, R.d_off_full, n_rec, total, R.d_counts, R.comp);
+            if (rc) return rc;
+            CK(cudaMemcpyAsync(h_counts, R.d_counts, n_rec * sizeof(uint32_t), cudaMemcpyDeviceToHost, R.comp));
+        }
+        if (h_hits) {
+            CK(cudaMemsetAsync(R.d_hits, 0, sizeof(unsigned long long), R.comp));
+            unsigned blocks = (unsigned)((n_bm + 255) / 256 < 1184 ? (n_bm + 255) / 256 : 1184);
+            count_total_kernel<<<blocks, 256, 0, R.comp>>>(R.d_bitmap, n_bm, R.d_hits);
+            CK(cudaGetLastError());
+            g_launches++;
+            CK(cudaMemcpyAsync(h_hits, R.d_hits, sizeof(uint64_t), cudaMemcpyDeviceToHost, R.comp));
+        }
+    }
+    CK(cudaStreamSynchronize(R.copy));
+    CK(cudaStreamSynchronize(R.comp));
+    return SBF_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int sbf_insert_seq_host(sbf_t *f, const char *h_seq, uint64_t len)
+{
+    if (!f || (!h_seq && len)) return fail(SBF_ERR_INVALID_ARG, "sbf_insert_seq_host: NULL argument");
+    return run_host(f, true, h_seq, nullptr, 0, len, nullptr, nullptr, nullptr);
+}
+
+int sbf_insert_records_host(sbf_t *f, const char *h_bases, const uint64_t *h_offsets, uint64_t n_rec)
+{
+    if (!f || !h_offsets) return fail(SBF_ERR_INVALID_ARG, "sbf_insert_records_host: NULL argument");
+    uint64_t total = h_offsets[n_rec];
+    if (!h_bases && total) return fail(SBF_ERR_INVALID_ARG, "sbf_insert_records_host: NULL bases");
+    return run_host(f, true, h_bases, h_offsets, n_rec, total, nullptr, nullptr, nullptr);
+}
+
+int sbf_query_seq_host(sbf_t *f, const char *h_seq, uint64_t len, uint32_t *h_bitmap, uint64_t *h_hits)
+{
+    if (!f || (!h_seq && len) || (!h_bitmap && len)) return fail(SBF_ERR_INVALID_ARG, "sbf_query_seq_host: NULL argument");
+    return run_host(f, false, h_seq, nullptr, 0, len, h_bitmap, nullptr, h_hits);
+}
+
+int sbf_query_records_host(sbf_t *f, const char *h_bases, const uint64_t *h_offsets, uint64_t n_rec, uint32_t *h_bitmap,
+                           uint32_t *h_hit_counts)
+{
+    if (!f || !h_offsets) return fail(SBF_ERR_INVALID_ARG, "sbf_query_records_host: NULL argument");
+    uint64_t total = h_offsets[n_rec];
+    if ((!h_bases || !h_bitmap) && total) return fail(SBF_ERR_INVALID_ARG, "sbf_query_records_host: NULL buffer");
+    return run_host(f, false, h_bases, h_offsets, n_rec, total, h_bitmap, h_hit_counts, nullptr);
+}
+
+} // extern "C"

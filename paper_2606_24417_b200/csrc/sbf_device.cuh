@@ -1,0 +1,545 @@
+// sbf_device.cuh — device code of the Super Bloom filter hot path (sm_100a).
+//
+// P:<n> = line n of the paper's extracted text; A<n> = reading n in DESIGN.md §3.
+// This file restates the pinned arithmetic on its own; it shares nothing with oracle/.
+//
+// Kernels
+//   pack_kernel        a1  ASCII -> 2-bit words (16 bases / uint32, first base in the top bits)
+//                          + "k-mer cannot start here" mask G (1 bit / base)
+//   mark_ends_kernel   a1  ORs the record-end bits into G
+//   stream_kernel      a2-a6  the fused, thread-serial streaming insert / query kernel
+//   naive_kernel       a2-a6  runtime-parameter one-k-mer-per-thread form of Alg. 1/2 (any legal k,m,s,H)
+//   count kernels      a6  per-record / total popcount of the result bitmap
+#pragma once
+
+#include <cstdint>
+#include <cuda_runtime.h>
+#include <type_traits>
+#include <utility>
+
+namespace sbfk {
+
+// ---- pinned constants (A1, A2, A4, A6) -------------------------------------------------
+constexpr uint64_t kSeedM = 0x5851F42D4C957F2Dull;
+constexpr uint32_t kMultG = 0x9E3779B1u;
+constexpr uint64_t kGold64 = 0x9E3779B97F4A7C15ull;
+constexpr uint64_t kSeedS = 0x2545F4914F6CDD1Dull;
+constexpr uint64_t kMultF = 0xD6E8FEB86659FD93ull;
+
+// ---- launch geometry ---------------------------------------------------------------------
+constexpr int kChunk = 128;     // k-mer start positions walked by one thread of stream_kernel
+constexpr int kStreamTPB = 128; // threads per CTA of stream_kernel
+constexpr int kPadWords = 16;   // zero / all-invalid words appended to the packed sequence and its mask
+
+struct StreamParams {
+    const uint32_t *packed; // 2-bit words, ceil(n_pos/16) + kPadWords
+    const uint16_t *gmask;  // one uint16 per packed word: bit j = G[16*word + j]
+    uint64_t n_pos;         // symbols in the batch (= k-mer start positions walked)
+    uint64_t *filter;       // 4 * numShards sector words
+    int shard_shift;        // 32 - P
+    uint32_t *bitmap;       // query: ceil(n_pos/32) words
+    uint64_t n_bitmap_words;
+};
+
+struct NaiveParams {
+    StreamParams sp;
+    int k, m, s, H;
+};
+
+__host__ __device__ constexpr uint64_t low_mask64(int nbits) { return nbits >= 64 ? ~0ull : ((1ull << nbits) - 1ull); }
+
+template <int I, int N, class F>
+__device__ __forceinline__ void static_for(F &&f)
+{
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        static_for<I + 1, N>(f);
+    }
+}
+
+// ---- the pinned primitives -----------------------------------------------------------------
+// A1: minimizer order key of an m-mer ("lightweight multiplicative hash")
+__device__ __forceinline__ uint32_t g_key(uint64_t x, int m)
+{
+    x ^= kSeedM & low_mask64(2 * m);
+    return ((uint32_t)x ^ (uint32_t)(x >> 32)) * kMultG;
+}
+// A2: minimizer key -> shard (power-of-two shard count, no division)
+__device__ __forceinline__ uint64_t sigma_shard(uint32_t key, int shard_shift)
+{
+    uint32_t t = (uint32_t)(((uint64_t)key * kGold64) >> 32);
+    return (uint64_t)t >> shard_shift;
+}
+// A4: s-mer hash ("stronger mix with an additional xorshift")
+__device__ __forceinline__ uint64_t f_hash(uint64_t x, int s)
+{
+    x ^= kSeedS & low_mask64(2 * s);
+    uint64_t h = (x ^ (x >> 28)) * kMultF;
+    return h ^ (h >> 32);
+}
+// A5 / A6: bit position of hash index i inside sector word i mod 4
+__device__ __forceinline__ int bit_pos(uint64_t h, int i, int H)
+{
+    int W = 64 / H;
+    if (W >= 6) return (int)((h >> (i * W)) & 63);
+    return (int)((h * ((uint64_t)(2 * i + 1) * kGold64)) >> 58);
+}
+
+__device__ __forceinline__ void ld_shard_256(const uint64_t *p, uint64_t (&w)[4])
+{
+    // one 256-bit non-coherent load per shard: LDG.E.ENL2.256.CONSTANT on sm_100a
+    asm volatile("ld.global.nc.v4.u64 {%0,%1,%2,%3}, [%4];" : "=l"(w[0]), "=l"(w[1]), "=l"(w[2]), "=l"(w[3]) : "l"(p));
+}
+
+__device__ __forceinline__ void red_or_64(uint64_t *p, uint64_t v)
+{
+    asm volatile("red.global.or.b64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+
+// =============================================================================================
+// a1: pack.  Thread i produces packed word i and mask word i from symbols [16i, 16i+16).
+//   code: A=0 C=1 G=2 T=3 (either case, A9); anything else is invalid (code bits arbitrary).
+//   B[j] = symbol j invalid or j >= len.   G[j] = B[j] | B[j+1] (k >= 2), = B[j] (k == 1).
+//   A k-mer starting at p is valid iff G[p .. p+max(k-1,1)-1] are all 0 once mark_ends_kernel
+//   has added F[j] = "a record ends after symbol j" (no k-mer spans records).
+// =============================================================================================
+__device__ __forceinline__ uint32_t pack4(uint32_t v, uint32_t &inv4)
+{
+    // four ASCII bytes (first symbol in the low byte) -> 8 bits, first symbol in the top 2 bits
+    uint32_t u = v & 0xDFDFDFDFu;
+    uint32_t ok = __vcmpeq4(u, 0x41414141u) | __vcmpeq4(u, 0x43434343u) | __vcmpeq4(u, 0x47474747u) |
+                  __vcmpeq4(u, 0x54545454u);
+    uint32_t x = (v >> 1) & 0x03030303u;
+    uint32_t c = x ^ ((x >> 1) & 0x01010101u);
+    inv4 = ((~ok & 0x01010101u) * 0x10204080u) >> 28; // bit j = symbol j invalid
+    return (c * 0x40100401u) >> 24;
+}
+
+#ifdef SBF_DEFINE_AUX_KERNELS // non-template kernels: defined in one translation unit (sbf_api.cu)
+__global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ seq, uint64_t len, uint32_t *__restrict__ packed,
+                                                   uint16_t *__restrict__ gmask, uint64_t n_words_total, int k, int aligned16)
+{
+    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint64_t b0 = i * 16;
+    uint32_t v[4];
+    if (aligned16 && b0 + 16 <= len) {
+        uint4 q = __ldg(reinterpret_cast<const uint4 *>(seq + b0));
+        v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+    } else {
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            uint32_t acc = 0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                uint64_t p = b0 + 4 * w + j;
+                uint32_t c = (p < len) ? (uint32_t)seq[p] : (uint32_t)'N';
+                acc |= c << (8 * j);
+            }
+            v[w] = acc;
+        }
+    }
+    uint32_t word = 0, inv = 0;
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        uint32_t i4;
+        uint32_t c8 = pack4(v[w], i4);
+        word |= c8 << (24 - 8 * w);
+        inv |= i4 << (4 * w);
+    }
+    // B of the next symbol: first flag of the next lane, or a direct byte load at the warp edge
+    uint32_t nxt = __shfl_down_sync(0xFFFFFFFFu, inv & 1u, 1);
+    if ((threadIdx.x & 31) == 31) {
+        uint64_t p = b0 + 16;
+        uint32_t c = (p < len) ? (uint32_t)seq[p] : (uint32_t)'N';
+        c &= 0xDFu;
+        nxt = !(c == 'A' || c == 'C' || c == 'G' || c == 'T');
+    }
+    uint32_t g = (k >= 2) ? (inv | (inv >> 1) | (nxt << 15)) : inv;
+    if (i < n_words_total) {
+        packed[i] = word;
+        gmask[i] = (uint16_t)g;
+    }
+}
+
+// F bits: a record boundary after symbol offsets[r]-1, r = 1..n_rec  (k >= 2 only)
+__global__ void mark_ends_kernel(const uint64_t *__restrict__ offsets, uint64_t n_rec, uint64_t total, uint32_t *gmask32)
+{
+    uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x + 1;
+    if (r > n_rec) return;
+    uint64_t e = offsets[r];
+    if (e == 0 || e > total) return;
+    uint64_t j = e - 1;
+    atomicOr(&gmask32[j >> 5], 1u << (j & 31));
+}
+
+#endif // SBF_DEFINE_AUX_KERNELS
+
+// =============================================================================================
+// Window access for stream_kernel.  W[0..2] hold 48 consecutive symbols (W[0] first, first symbol
+// in the top bits).  lmer<O,N>(W) = the N-mer starting O symbols into the window, as Sub() of the
+// paper's packed k-mer (first base most significant).  All shifts are immediates.
+// =============================================================================================
+template <int Q, int NB>
+__device__ __forceinline__ uint32_t field96(const uint32_t (&W)[3])
+{
+    static_assert(Q >= 0 && NB >= 1 && NB <= 32 && Q + NB <= 96, "field outside the 96-bit window");
+    constexpr int idx = Q / 32, sh = Q % 32;
+    uint32_t lo = W[2 - idx];
+    uint32_t v;
+    if constexpr (sh == 0) {
+        v = lo;
+    } else if constexpr (sh + NB <= 32) {
+        v = lo >> sh;
+    } else {
+        v = __funnelshift_r(lo, W[1 - idx], sh);
+    }
+    if constexpr (NB < 32 && !(sh + NB == 32)) v &= (1u << NB) - 1u;
+    return v;
+}
+
+template <int O, int N>
+__device__ __forceinline__ uint64_t lmer(const uint32_t (&W)[3])
+{
+    constexpr int Q = 96 - 2 * O - 2 * N;
+    constexpr int nb = 2 * N;
+    uint32_t lo = field96<Q, (nb < 32 ? nb : 32)>(W);
+    uint32_t hi = 0;
+    if constexpr (nb > 32) hi = field96<Q + 32, nb - 32>(W);
+    return ((uint64_t)hi << 32) | lo;
+}
+
+__device__ __forceinline__ uint32_t min3u(uint32_t a, uint32_t b, uint32_t c) { return min(min(a, b), c); }
+
+// Sliding minimum of the last WN keys, streaming: keys arrive one per step, E = step phase (mod 16
+// is all that matters).  Levels c3 = min of the last 3, c9 = min of the last 9; the window of WN is
+// covered by two or three overlapping blocks (three-input minimum = VIMNMX3 on sm_100a).
+template <int WN>
+struct SlidingMin {
+    static_assert(WN >= 1 && WN <= 24, "stream kernel supports k-m+1 <= 24");
+    uint32_t g[16], c3[16], c9[16];
+    template <int E>
+    __device__ __forceinline__ uint32_t push(uint32_t gn)
+    {
+        constexpr int s0 = E & 15;
+        g[s0] = gn;
+        if constexpr (WN == 1) return gn;
+        if constexpr (WN == 2) return min(gn, g[(E - 1) & 15]);
+        uint32_t a3 = min3u(gn, g[(E - 1) & 15], g[(E - 2) & 15]);
+        c3[s0] = a3;
+        if constexpr (WN == 3) return a3;
+        if constexpr (WN >= 4 && WN <= 6) return min(a3, c3[(E - (WN - 3)) & 15]);
+        if constexpr (WN >= 7 && WN <= 9) return min3u(a3, c3[(E - 3) & 15], c3[(E - (WN - 3)) & 15]);
+        if constexpr (WN >= 10) {
+            uint32_t a9 = min3u(a3, c3[(E - 3) & 15], c3[(E - 6) & 15]);
+            c9[s0] = a9;
+            if constexpr (WN <= 18) return min(a9, c9[(E - (WN - 9)) & 15]);
+            else return min3u(a9, c9[(E - 9) & 15], c9[(E - (WN - 9)) & 15]);
+        }
+        return gn;
+    }
+};
+
+// One-hot sector masks of one s-mer hash: hash index i -> word i mod 4, bit B(h,i) (A5)
+template <int H, int NW>
+__device__ __forceinline__ void expand_masks(uint64_t h, uint64_t (&m)[NW])
+{
+    constexpr int Wd = 64 / H;
+    static_assert(Wd >= 6, "bit-slicing needs 64/H >= 6");
+#pragma unroll
+    for (int q = 0; q < NW; ++q) m[q] = 0;
+    static_for<0, H>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        m[i & 3] |= 1ull << ((h >> (i * Wd)) & 63);
+    });
+}
+
+__host__ __device__ constexpr int ring_size(int z) { return z <= 1 ? 1 : z <= 2 ? 2 : z <= 4 ? 4 : z <= 8 ? 8 : 16; }
+
+// =============================================================================================
+// a2-a6 fused.  One thread walks kChunk consecutive k-mer start positions p0 .. p0+kChunk-1 of the
+// batch, carrying in registers: the 48-symbol window, the sliding-minimum rings (a2), the one-hot
+// masks of the last k-s s-mers, and
+//   insert: the OR of the current super-k-mer's masks (a5), flushed with one RED.OR.B64 per sector
+//           word when the minimizer key (hence the shard, A14) or validity changes;
+//   query : the current shard's 256 bits (a6), reloaded when the key changes; the k-mer's mask
+//           K = OR of its k-s+1 s-mer masks is tested with K & ~shard == 0 (Findere rule).
+// Each m-mer key and each s-mer hash is computed once per position (not once per k-mer as in
+// Alg. 1/2); the result bits are the same because OR/AND do not care about order or repetition.
+// =============================================================================================
+template <int K, int M, int S, int H, bool INSERT>
+__global__ void __launch_bounds__(kStreamTPB) stream_kernel(const StreamParams prm)
+{
+    constexpr int WN = K - M + 1;
+    constexpr int Z = K - S;
+    constexpr int NW = H < 4 ? H : 4;
+    constexpr int RZ = ring_size(Z);
+    constexpr int L = K > 1 ? K - 1 : 1;
+    constexpr uint32_t maskL = (L >= 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
+    static_assert(K >= 1 && K <= 32 && M >= 1 && M <= K && S >= 1 && S <= K, "bad k/m/s");
+    static_assert(Z <= 16, "stream kernel supports k-s <= 16");
+
+    const uint64_t chunk = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint64_t p0 = chunk * kChunk;
+    if (p0 >= prm.n_pos) return;
+
+    const uint32_t *__restrict__ pw = prm.packed + (p0 >> 4);
+    const uint16_t *__restrict__ gw = prm.gmask + (p0 >> 4);
+    uint32_t W[3] = {__ldg(pw), __ldg(pw + 1), __ldg(pw + 2)};
+    uint32_t glo = (uint32_t)__ldg(gw) | ((uint32_t)__ldg(gw + 1) << 16);
+    uint32_t ghi = __ldg(gw + 2);
+
+    SlidingMin<WN> smin;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { smin.g[i] = 0; smin.c3[i] = 0; smin.c9[i] = 0; }
+    uint64_t Mh[RZ][NW];
+#pragma unroll
+    for (int i = 0; i < RZ; ++i)
+#pragma unroll
+        for (int q = 0; q < NW; ++q) Mh[i][q] = 0;
+
+    // prologue: keys of the first WN-1 m-mers, masks of the first Z s-mers
+    static_for<0, WN - 1>([&](auto ec) {
+        constexpr int E = decltype(ec)::value;
+        (void)smin.template push<E>(g_key(lmer<E, M>(W), M));
+    });
+    static_for<0, Z>([&](auto ic) {
+        constexpr int I = decltype(ic)::value;
+        expand_masks<H, NW>(f_hash(lmer<I, S>(W), S), Mh[I % RZ]);
+    });
+
+    uint64_t acc[NW];   // insert: OR of the current run's masks
+    uint64_t shard[4];  // query: the current shard's sector words
+#pragma unroll
+    for (int q = 0; q < NW; ++q) acc[q] = 0;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) shard[q] = 0;
+    uint32_t prevKey = 0;
+    bool prevInval = true; // insert: previous k-mer invalid; query: no shard loaded yet
+    uint32_t res = 0;
+
+    for (int b = 0; b < kChunk / 16; ++b) {
+        const uint32_t wnext = __ldg(pw + b + 3);
+        const uint32_t gnext = __ldg(gw + b + 3);
+        uint32_t res16 = 0;
+        static_for<0, 16>([&](auto jc) {
+            constexpr int J = decltype(jc)::value;
+            // a2: key of the newest m-mer of k-mer p = p0+16b+J, then the window minimum
+            const uint32_t key = smin.template push<J + WN - 1>(g_key(lmer<J + WN - 1, M>(W), M));
+            // a4: the newest s-mer of that k-mer
+            uint64_t Mn[NW];
+            expand_masks<H, NW>(f_hash(lmer<J + Z, S>(W), S), Mn);
+            // a1: validity of k-mer p
+            const bool inval = (__funnelshift_r(glo, ghi, J) & maskL) != 0;
+            if constexpr (INSERT) {
+                const bool brk = (key != prevKey) || (inval != prevInval);
+                if (brk) {
+                    if (!prevInval) { // a5: flush the finished run
+                        uint64_t *dst = prm.filter + sigma_shard(prevKey, prm.shard_shift) * 4;
+#pragma unroll
+                        for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
+                    }
+#pragma unroll
+                    for (int q = 0; q < NW; ++q) { // restart with the k-s s-mers shared with the previous k-mers
+                        uint64_t r = 0;
+#pragma unroll
+                        for (int i = 0; i < Z; ++i) r |= Mh[(J + i) % RZ][q];
+                        acc[q] = r;
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < NW; ++q) acc[q] |= Mn[q];
+                prevKey = key;
+                prevInval = inval;
+            } else {
+                const bool need = !inval && (prevInval || key != prevKey);
+                if (need) { // a6: fetch the shard of the new run
+                    ld_shard_256(prm.filter + sigma_shard(key, prm.shard_shift) * 4, shard);
+                    prevKey = key;
+                    prevInval = false;
+                }
+                uint64_t miss = 0;
+#pragma unroll
+                for (int q = 0; q < NW; ++q) {
+                    uint64_t kq = Mn[q];
+#pragma unroll
+                    for (int i = 0; i < Z; ++i) kq |= Mh[(J + i) % RZ][q];
+                    miss |= kq & ~shard[q];
+                }
+                if (!inval && miss == 0) res16 |= 1u << J;
+            }
+#pragma unroll
+            for (int q = 0; q < NW; ++q) Mh[(J + Z) % RZ][q] = Mn[q];
+        });
+        W[0] = W[1]; W[1] = W[2]; W[2] = wnext;
+        glo = (glo >> 16) | (ghi << 16);
+        ghi = gnext;
+        if constexpr (!INSERT) {
+            res = (res >> 16) | (res16 << 16);
+            if (b & 1) {
+                const uint64_t wi = (p0 >> 5) + (uint64_t)(b >> 1);
+                if (wi < prm.n_bitmap_words) prm.bitmap[wi] = res;
+            }
+        }
+    }
+    if constexpr (INSERT) {
+        if (!prevInval) {
+            uint64_t *dst = prm.filter + sigma_shard(prevKey, prm.shard_shift) * 4;
+#pragma unroll
+            for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
+        }
+    }
+}
+
+// =============================================================================================
+// Runtime-parameter kernel: Alg. 1 / Alg. 2 as printed, one k-mer per thread, everything
+// recomputed per k-mer.  Serves every legal (k,m,s,H) that has no
+// specialised instance, including H > 10 (A6).  A warp covers 32 consecutive positions, so the
+// query result word is one ballot.
+// =============================================================================================
+__device__ __forceinline__ uint64_t load_kmer(const uint32_t *__restrict__ packed, uint64_t p, int k)
+{
+    const uint32_t *w = packed + (p >> 4);
+    uint32_t a = __ldg(w), b = __ldg(w + 1), c = __ldg(w + 2);
+    int sh = 2 * (int)(p & 15);
+    uint32_t hi = __funnelshift_l(b, a, sh); // symbols p .. p+15
+    uint32_t lo = __funnelshift_l(c, b, sh); // symbols p+16 .. p+31
+    uint64_t v = ((uint64_t)hi << 32) | lo;
+    return v >> (64 - 2 * k);
+}
+
+__device__ __forceinline__ bool kmer_invalid(const uint16_t *__restrict__ gmask, uint64_t p, int k)
+{
+    const uint16_t *g = gmask + (p >> 4);
+    uint64_t bits = (uint64_t)__ldg(g) | ((uint64_t)__ldg(g + 1) << 16) | ((uint64_t)__ldg(g + 2) << 32);
+    int L = k > 1 ? k - 1 : 1;
+    return ((bits >> (p & 15)) & low_mask64(L)) != 0;
+}
+
+template <bool INSERT>
+__global__ void __launch_bounds__(256) naive_kernel(const NaiveParams np)
+{
+    const StreamParams &prm = np.sp;
+    const int k = np.k, m = np.m, s = np.s, H = np.H;
+    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; // grid covers a multiple of 32 positions
+    bool present = false;
+    if (p < prm.n_pos && !kmer_invalid(prm.gmask, p, k)) {
+        const uint64_t v = load_kmer(prm.packed, p, k);
+        uint32_t minKey = 0xFFFFFFFFu;
+        for (int i = 0; i <= k - m; ++i) { // Alg. 1 l.5-9
+            uint64_t x = (v >> (2 * (k - m - i))) & low_mask64(2 * m);
+            minKey = min(minKey, g_key(x, m));
+        }
+        uint64_t *sh = prm.filter + sigma_shard(minKey, prm.shard_shift) * 4;
+        uint64_t w[4] = {0, 0, 0, 0};
+        if constexpr (!INSERT) ld_shard_256(sh, w);
+        uint64_t mk[4] = {0, 0, 0, 0};
+        for (int j = 0; j <= k - s; ++j) { // Alg. 1 l.11-14 / Alg. 2 Contains
+            uint64_t x = (v >> (2 * (k - s - j))) & low_mask64(2 * s);
+            uint64_t h = f_hash(x, s);
+            for (int i = 0; i < H; ++i) {
+                uint64_t bit = 1ull << bit_pos(h, i, H);
+                switch (i & 3) {
+                case 0: mk[0] |= bit; break;
+                case 1: mk[1] |= bit; break;
+                case 2: mk[2] |= bit; break;
+                default: mk[3] |= bit; break;
+                }
+            }
+        }
+        if constexpr (INSERT) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (mk[q]) red_or_64(sh + q, mk[q]);
+        } else {
+            present = ((mk[0] & ~w[0]) | (mk[1] & ~w[1]) | (mk[2] & ~w[2]) | (mk[3] & ~w[3])) == 0;
+        }
+    }
+    if constexpr (!INSERT) {
+        uint32_t word = __ballot_sync(0xFFFFFFFFu, present);
+        if ((threadIdx.x & 31) == 0) {
+            uint64_t wi = p >> 5;
+            if (wi < prm.n_bitmap_words) prm.bitmap[wi] = word;
+        }
+    }
+}
+
+// =============================================================================================
+// a6: hit counts from the result bitmap.
+// =============================================================================================
+__device__ __forceinline__ uint32_t popc_range(const uint32_t *__restrict__ bm, uint64_t a, uint64_t e)
+{
+    // set bits in bit positions [a, e)
+    if (a >= e) return 0;
+    uint64_t wa = a >> 5, we = (e - 1) >> 5;
+    uint32_t first = 0xFFFFFFFFu << (a & 31);
+    uint32_t last = 0xFFFFFFFFu >> (31 - ((e - 1) & 31));
+    if (wa == we) return __popc(__ldg(bm + wa) & first & last);
+    uint32_t c = __popc(__ldg(bm + wa) & first) + __popc(__ldg(bm + we) & last);
+    for (uint64_t w = wa + 1; w < we; ++w) c += __popc(__ldg(bm + w));
+    return c;
+}
+
+#ifdef SBF_DEFINE_AUX_KERNELS
+// short records: one thread per record
+__global__ void __launch_bounds__(256) count_records_thread_kernel(const uint32_t *__restrict__ bm, const uint64_t *__restrict__ offsets,
+                                                                   uint64_t n_rec, uint32_t *__restrict__ counts)
+{
+    uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= n_rec) return;
+    counts[r] = popc_range(bm, offsets[r], offsets[r + 1]);
+}
+
+// long records: one CTA per record, grid-stride over records
+__global__ void __launch_bounds__(256) count_records_block_kernel(const uint32_t *__restrict__ bm, const uint64_t *__restrict__ offsets,
+                                                                  uint64_t n_rec, uint32_t *__restrict__ counts)
+{
+    __shared__ uint32_t part[8];
+    for (uint64_t r = blockIdx.x; r < n_rec; r += gridDim.x) {
+        uint64_t a = offsets[r], e = offsets[r + 1];
+        uint32_t c = 0;
+        // split [a,e) in 32-aligned pieces, one per thread per round
+        uint64_t a32 = a & ~31ull;
+        for (uint64_t w = a32 + 32ull * threadIdx.x; w < e; w += 32ull * blockDim.x) {
+            uint64_t lo = w < a ? a : w, hi = (w + 32 < e) ? w + 32 : e;
+            c += popc_range(bm, lo, hi);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, o);
+        if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = c;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            uint32_t t = 0;
+            for (int i = 0; i < (int)(blockDim.x >> 5); ++i) t += part[i];
+            counts[r] = t;
+        }
+        __syncthreads();
+    }
+}
+
+// total popcount of n_words words -> *hits (must be zeroed before)
+__global__ void __launch_bounds__(256) count_total_kernel(const uint32_t *__restrict__ bm, uint64_t n_words, unsigned long long *hits)
+{
+    unsigned long long c = 0;
+    for (uint64_t w = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; w < n_words; w += (uint64_t)gridDim.x * blockDim.x)
+        c += __popc(__ldg(bm + w));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, o);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(hits, c);
+}
+
+// filter |= src  (replica merge)
+__global__ void __launch_bounds__(256) or_words_kernel(uint64_t *__restrict__ dst, const uint64_t *__restrict__ src, uint64_t n_words)
+{
+    uint64_t n2 = n_words / 2;
+    ulonglong2 *d2 = reinterpret_cast<ulonglong2 *>(dst);
+    const ulonglong2 *s2 = reinterpret_cast<const ulonglong2 *>(src);
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (uint64_t)gridDim.x * blockDim.x) {
+        ulonglong2 a = d2[i], b = s2[i];
+        a.x |= b.x; a.y |= b.y;
+        d2[i] = a;
+    }
+}
+
+#endif // SBF_DEFINE_AUX_KERNELS
+
+} // namespace sbfk

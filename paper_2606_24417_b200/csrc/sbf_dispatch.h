@@ -1,0 +1,39 @@
+// sbf_dispatch.h — table of specialised stream_kernel instances, filled by the sbf_inst_*.cu files.
+#pragma once
+
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "sbf_device.cuh"
+
+namespace sbfk {
+
+typedef cudaError_t (*stream_launch_fn)(const StreamParams &prm, cudaStream_t stream);
+
+struct KernelEntry {
+    int k, m, s, H;
+    stream_launch_fn insert;
+    stream_launch_fn query;
+};
+
+template <int K, int M, int S, int H, bool INSERT>
+cudaError_t launch_stream(const StreamParams &prm, cudaStream_t stream)
+{
+    const uint64_t chunks = (prm.n_pos + kChunk - 1) / kChunk;
+    if (chunks == 0) return cudaSuccess;
+    const uint64_t blocks = (chunks + kStreamTPB - 1) / kStreamTPB;
+    stream_kernel<K, M, S, H, INSERT><<<(unsigned)blocks, kStreamTPB, 0, stream>>>(prm);
+    return cudaGetLastError();
+}
+
+#define SBF_ENTRY(K, M, S, H) \
+    { K, M, S, H, &sbfk::launch_stream<K, M, S, H, true>, &sbfk::launch_stream<K, M, S, H, false> }
+
+// one table per translation unit (compiled in parallel)
+const KernelEntry *inst_table_default(int *n);
+const KernelEntry *inst_table_s_axis(int *n);
+const KernelEntry *inst_table_m_axis(int *n);
+const KernelEntry *inst_table_h_axis(int *n);
+const KernelEntry *inst_table_small(int *n);
+
+} // namespace sbfk
