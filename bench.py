@@ -1,0 +1,522 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the Super Bloom filter insert + query hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload config3]
+
+One STEP = one pass of the whole hot path over one batch of the
+workload: clear the filter, insert the workload's sequence (pack -> fused minimizer / shard /
+s-mer / merge kernel), [N>1: OR all-reduce of the replicas], query one batch of reads (pack ->
+fused query kernel -> packed bitmap -> per-record hit counts).  `value` = valid k-mers inserted
++ valid k-mers queried by all ranks, per second of device time (max over ranks).
+
+Default workload: BASELINE.json configs[2] (the out-of-L2 config north_star's target is quoted
+on): 250 Mbp order-5 Markov sequence with N runs, k=31 m=16 s=28 H=4, filter 2^32 bits; reads of
+length 150 (half sampled with 1% substitutions, half uniform), queried in batches.  All inputs are
+seeded synthetic stand-ins (seqgen/), see DESIGN.md "Input recipe".
+
+The product path is the C ABI (include/sbf.h) through its ctypes binding; the oracle is executed
+only by the `cpu_baseline` leg and by `--impl reference`.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "G k-mers/s insert+query (1 step = insert the sequence + query one read batch)"
+# algorithmic work per valid k-mer, defaults k=31 m=16 s=28 H=4
+OPS_PER_KMER = {"insert": 70.0, "query": 63.0}          # integer lane-ops
+# ALU peak derived in DESIGN.md §6: 148 SMs x 4 SMSPs x 16 lanes/clk (alu pipe, rt=2) x max SM clock
+ALU_LANES_PER_CLK = 148 * 4 * 16
+
+
+def env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        return float(d.get("hbm_gbs", 6650.0)), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+# ------------------------------------------------------------------------------------------------
+# workload
+# ------------------------------------------------------------------------------------------------
+def make_workload(name: str, rank: int, scale: float):
+    import seqgen
+    if name == "config3":
+        w = seqgen.config3(scale=scale)
+    elif name == "config2":
+        w = seqgen.config2(scale=scale)
+        w.params["num_bits"] = 1 << 27
+    elif name == "config1":
+        w = seqgen.config1()
+        w.n_reads = 6000
+        w.read_seed = 3
+    else:
+        raise SystemExit("unknown workload %r" % name)
+    if rank:  # weak scaling: every rank owns an independent sequence of the same recipe
+        n = w.insert_bases.size
+        if name == "config3":
+            seq = seqgen.markov(31 + 1000 * rank, 5, 0.41, n)
+            seqgen.plant_n_runs(32 + 1000 * rank, seq, max(1, int(round(100 * scale))), 10_000, 50_000)
+        elif name == "config2":
+            seq = seqgen.markov(21 + 1000 * rank, 3, 0.50, n)
+            seqgen.plant_copies(22 + 1000 * rank, seq, max(1, int(200 * scale)), 1000, 5000, 0.005)
+        else:
+            seq = seqgen.uniform(1 + 1000 * rank, n)
+        w.insert_bases = seq
+        w.read_seed += 1000 * rank
+    return w
+
+
+_ACGT = np.zeros(256, dtype=bool)
+for _c in b"ACGTacgt":
+    _ACGT[_c] = True
+
+
+def count_valid_kmers_seq(seq: np.ndarray, k: int) -> int:
+    """k-mer windows of one sequence without a non-ACGT symbol (harness bookkeeping for the metric)."""
+    n = seq.size
+    if n < k:
+        return 0
+    total, step = 0, 1 << 26
+    for a in range(0, n - k + 1, step):
+        e = min(a + step + k - 1, n)
+        bad = ~_ACGT[seq[a:e]]
+        if not bad.any():
+            total += e - a - k + 1
+            continue
+        cs = np.concatenate(([0], np.cumsum(bad, dtype=np.int32)))
+        total += int(np.count_nonzero(cs[k:] - cs[:-k] == 0))
+    return total
+
+
+def count_valid_kmers_reads(reads: np.ndarray, read_len: int, k: int) -> int:
+    n = reads.size // read_len
+    per = max(read_len - k + 1, 0)
+    bad_rows = np.flatnonzero((~_ACGT[reads]).reshape(n, read_len).any(axis=1))
+    total = (n - bad_rows.size) * per
+    for r in bad_rows:
+        total += count_valid_kmers_seq(reads[r * read_len:(r + 1) * read_len], k)
+    return total
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS, "--format=csv,noheader,nounits",
+                 "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append((time.perf_counter(), ln.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for t, ln in self.lines:
+            if t < t0 or t > t1 + 0.06:
+                continue
+            parts = [x.strip() for x in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:  # region shorter than the sampling period: take whatever was seen
+            for t, ln in self.lines[-3:]:
+                parts = [x.strip() for x in ln.split(",")]
+                try:
+                    sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+                except (ValueError, IndexError):
+                    pass
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------
+# the oracle on the host cores (cpu_baseline leg and --impl reference): bounded sample
+# ------------------------------------------------------------------------------------------------
+def oracle_sample_step(o, seq_sample, reads_sample, offs_sample, threads: bool):
+    """One oracle 'step' on the bounded sample: clear, insert, query.  Returns (k-mers, seconds)."""
+    t0 = time.perf_counter()
+    o.clear()
+    n_ins = o.insert_records(seq_sample, threads=threads)
+    t1 = time.perf_counter()
+    _, _, n_q = o.query_records(reads_sample, offs_sample, want_counts=True, threads=threads)
+    t2 = time.perf_counter()
+    return n_ins, n_q, t1 - t0, t2 - t1
+
+
+def make_oracle_sample(w, ins_bases: int, n_reads: int):
+    import seqgen
+    seq_sample = np.ascontiguousarray(w.insert_bases[:ins_bases])
+    reads_sample = w.read_batch(0, n_reads)
+    offs = seqgen.fixed_offsets(n_reads, w.read_len)
+    return seq_sample, reads_sample, offs
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands, all host cores (its OpenMP driver), bounded sample."""
+    rank = env_int("RANK", 0)
+    if rank != 0:
+        return 0
+    import oracle
+    w = make_workload(args.workload, 0, args.ref_scale)
+    p = w.params
+    ins_bases = min(w.insert_bases.size, args.ref_insert_bases)
+    n_reads = min(max(w.n_reads, 1), args.ref_reads)
+    seq_s, reads_s, offs_s = make_oracle_sample(w, ins_bases, n_reads)
+    o = oracle.OracleSBF(p["k"], p["m"], p["s"], p["H"], p["num_bits"])
+    cores = oracle.num_threads()
+    for _ in range(args.warmup):
+        oracle_sample_step(o, seq_s, reads_s, offs_s, True)
+    kmers, secs, ti, tq, ni, nq = 0, 0.0, 0.0, 0.0, 0, 0
+    for _ in range(args.steps):
+        a, b, t_i, t_q = oracle_sample_step(o, seq_s, reads_s, offs_s, True)
+        kmers += a + b; secs += t_i + t_q; ti += t_i; tq += t_q; ni += a; nq += b
+    val = kmers / secs / 1e9
+    sample = "per step: insert first %d bases of the %s sequence + query first %d reads x %d" % (
+        ins_bases, args.workload, n_reads, w.read_len)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val,
+        "unit": "G k-mers/s", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": secs / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u64", "data": "synthetic",
+        "config": {"workload": args.workload, "k": p["k"], "m": p["m"], "s": p["s"], "H": p["H"],
+                   "filter_bits": o.num_bits, "sample": sample},
+        "insert_gkmers_s": ni / ti / 1e9, "query_gkmers_s": nq / tq / 1e9,
+        "cpu_baseline": {"value": val, "unit": "G k-mers/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": "G k-mers/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+    import seqgen
+    import paper_2606_24417_b200 as sbf
+    from paper_2606_24417_b200 import replicas
+
+    world = env_int("WORLD_SIZE", 1)
+    rank = env_int("RANK", 0)
+    local_rank = env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — this framework has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    sbf.load_library(build_if_missing=True)
+    hbm_gbs, sm_max_mhz, peak_src = load_peaks()
+
+    # ---- inputs (host, pinned) -> device -------------------------------------------------------
+    w = make_workload(args.workload, rank, args.scale)
+    p = w.params
+    k = p["k"]
+    seq_h = torch.from_numpy(w.insert_bases).pin_memory()
+    n_ins_kmers = count_valid_kmers_seq(w.insert_bases, k)
+    rb = min(args.read_batch, max(w.n_reads, 1))
+    n_batches = max(1, min(args.batches, max(w.n_reads, 1) // rb))
+    offs_np = seqgen.fixed_offsets(rb, w.read_len)
+    reads_h, n_q_kmers = [], []
+    for b in range(n_batches):
+        t = torch.empty(rb * w.read_len, dtype=torch.uint8).pin_memory()
+        w.read_batch(b * rb, rb, out=t.numpy())
+        reads_h.append(t)
+        n_q_kmers.append(count_valid_kmers_reads(t.numpy(), w.read_len, k))
+    offs_h = torch.from_numpy(offs_np.view(np.int64)).pin_memory()
+
+    d_seq = seq_h.cuda(non_blocking=True)
+    d_reads = [t.cuda(non_blocking=True) for t in reads_h]
+    d_offs = offs_h.cuda(non_blocking=True)
+    n_read_bases = rb * w.read_len
+    d_bitmap = torch.empty((n_read_bases + 31) // 32, dtype=torch.int32, device="cuda")
+    d_counts = torch.empty(rb, dtype=torch.int32, device="cuda")
+    h_bitmap = torch.empty((n_read_bases + 31) // 32, dtype=torch.int32).pin_memory()
+    h_counts = torch.empty(rb, dtype=torch.int32).pin_memory()
+    torch.cuda.synchronize()
+
+    h = sbf.sbf_create(k, p["m"], p["s"], p["H"], p["num_bits"])
+    num_bits = sbf.sbf_num_bits(h)
+    sbf.sbf_reserve(h, max(d_seq.numel(), n_read_bases))
+    sbf.sbf_set_timing(h, True)
+    stream = torch.cuda.current_stream()
+
+    def step(i: int, ev=None):
+        b = i % n_batches
+        if ev: ev[0].record(stream)
+        sbf.sbf_clear(h, stream)
+        sbf.sbf_insert_seq(h, d_seq, d_seq.numel(), stream)
+        if world > 1:
+            replicas.or_allreduce_filter(h, stream=stream)
+        if ev: ev[1].record(stream)
+        sbf.sbf_query_records(h, d_reads[b], d_offs, rb, n_read_bases, d_bitmap, d_counts, stream)
+        if ev: ev[2].record(stream)
+        return b
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up, then the timed region ----------------------------------------------------------
+    for i in range(args.warmup):
+        step(i)
+    barrier()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    ins_kernel_ms, q_kernel_ms, pack_ms, count_ms = [], [], [], []
+    sampler = ClockSampler(local_rank if "CUDA_VISIBLE_DEVICES" not in os.environ else
+                           int(os.environ["CUDA_VISIBLE_DEVICES"].split(",")[local_rank]))
+    sampler.start()
+    time.sleep(0.12)
+    launches0 = sbf.sbf_kernel_launches()
+    barrier()
+    t_host0 = time.perf_counter()
+    e_begin = torch.cuda.Event(enable_timing=True); e_end = torch.cuda.Event(enable_timing=True)
+    e_begin.record(stream)
+    q_total = 0
+    for i in range(args.steps):
+        b = step(args.warmup + i, evs[i])
+        q_total += n_q_kmers[b]
+    e_end.record(stream)
+    barrier()
+    t_host1 = time.perf_counter()
+    launches = sbf.sbf_kernel_launches() - launches0
+    clocks = sampler.stop(t_host0, t_host1)
+    total_ms = e_begin.elapsed_time(e_end)
+    ins_ms = sum(e[0].elapsed_time(e[1]) for e in evs)
+    qry_ms = sum(e[1].elapsed_time(e[2]) for e in evs)
+
+    # per-kernel device times (events the library records on the same stream around each kernel):
+    # a few extra steps, same inputs, so that the two calls of a step can be read separately
+    for i in range(min(args.steps, 5)):
+        b = (args.warmup + i) % n_batches
+        sbf.sbf_clear(h, stream)
+        sbf.sbf_insert_seq(h, d_seq, d_seq.numel(), stream)
+        pk, mn, _ = sbf.sbf_get_timing(h)
+        ins_kernel_ms.append(mn); pack_ms.append(pk)
+        sbf.sbf_query_records(h, d_reads[b], d_offs, rb, n_read_bases, d_bitmap, d_counts, stream)
+        pk, mn, ct = sbf.sbf_get_timing(h)
+        q_kernel_ms.append((mn, n_q_kmers[b])); pack_ms.append(pk); count_ms.append(ct)
+    torch.cuda.synchronize()
+
+    # measured statistics of the last query batch: FPR on the uniform reads (odd read index)
+    cnt = d_counts.cpu().numpy().view(np.uint32).astype(np.int64)
+    per_read = max(w.read_len - k + 1, 1)
+    fpr_random = float(cnt[1::2].sum()) / max(1, cnt[1::2].size * per_read)
+    hit_sampled = float(cnt[0::2].sum()) / max(1, cnt[0::2].size * per_read)
+
+    # ---- end to end through the host-facing C ABI (pinned host buffers, H2D + D2H inside) -----------
+    sbf.sbf_set_timing(h, False)
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    hb_np, hc_np = h_bitmap.numpy().view(np.uint32), h_counts.numpy().view(np.uint32)
+
+    def e2e_step(i):
+        b = i % n_batches
+        sbf.sbf_clear(h, None)
+        sbf.sbf_insert_seq_host(h, seq_h, seq_h.numel())
+        if world > 1:
+            replicas.or_allreduce_filter(h, stream=stream)
+            torch.cuda.synchronize()
+        sbf.sbf_query_records_host(h, reads_h[b], offs_np, rb, hb_np, hc_np)
+        return b
+
+    e2e_step(0)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_kmers = 0
+    for i in range(e2e_steps):
+        b = e2e_step(i + 1)
+        e2e_kmers += n_ins_kmers + n_q_kmers[b]
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    h2d = seq_h.numel() + n_read_bases + offs_np.nbytes
+    d2h = hb_np.nbytes + hc_np.nbytes
+
+    # ---- reduce over ranks ------------------------------------------------------------------------
+    kmers_local = args.steps * n_ins_kmers + q_total
+    vals = torch.tensor([total_ms, ins_ms, qry_ms, e2e_s, float(kmers_local), float(e2e_kmers),
+                         float(args.steps * n_ins_kmers), float(q_total)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        mx = vals.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+        sm = vals.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+        total_ms, ins_ms, qry_ms, e2e_s = (float(x) for x in mx[:4])
+        kmers_all, e2e_kmers_all, ins_all, q_all = (float(x) for x in sm[4:])
+    else:
+        kmers_all, e2e_kmers_all, ins_all, q_all = float(kmers_local), float(e2e_kmers), float(
+            args.steps * n_ins_kmers), float(q_total)
+
+    if rank == 0:
+        value = kmers_all / (total_ms * 1e-3) / 1e9
+        ins_rate = ins_all / (ins_ms * 1e-3) / 1e9
+        q_rate = q_all / (qry_ms * 1e-3) / 1e9
+        # rooflines.  ALU: algorithmic lane-ops / kernel time vs the alu-pipe peak at max clock.
+        alu_peak = ALU_LANES_PER_CLK * sm_max_mhz * 1e6 / 1e12          # T lane-ops/s
+        ik = statistics.mean(ins_kernel_ms)
+        qk = statistics.mean(m for m, _ in q_kernel_ms)
+        qk_kmers = statistics.mean(n for _, n in q_kernel_ms)
+        w_ = k - p["m"] + 1
+        d_runs = 2.0 / (w_ + 1)
+        # HBM: algorithmic bytes of the fused kernels (packed 2-bit words + mask + one sector read/write per run)
+        ins_bytes = d_seq.numel() * (0.25 + 0.125) + n_ins_kmers * d_runs * 64.0
+        q_bytes = n_read_bases * (0.25 + 0.125 + 0.125) + qk_kmers * (d_runs + 1.0 / per_read) * 32.0
+        roof = {
+            "insert_kernel": {"bound": "alu", "achieved": OPS_PER_KMER["insert"] * n_ins_kmers / (ik * 1e-3) / 1e12,
+                              "peak": alu_peak, "unit": "Tiop/s", "ms": ik, "gkmers_s": n_ins_kmers / ik / 1e6,
+                              "hbm_gbs_algorithmic": ins_bytes / (ik * 1e-3) / 1e9},
+            "query_kernel": {"bound": "alu", "achieved": OPS_PER_KMER["query"] * qk_kmers / (qk * 1e-3) / 1e12,
+                             "peak": alu_peak, "unit": "Tiop/s", "ms": qk, "gkmers_s": qk_kmers / qk / 1e6,
+                             "hbm_gbs_algorithmic": q_bytes / (qk * 1e-3) / 1e9},
+            "pack_kernel_ms_mean": statistics.mean(pack_ms), "count_kernel_ms_mean": statistics.mean(count_ms),
+        }
+        for kk in ("insert_kernel", "query_kernel"):
+            roof[kk]["frac"] = roof[kk]["achieved"] / roof[kk]["peak"]
+            roof[kk]["hbm_frac"] = roof[kk]["hbm_gbs_algorithmic"] / hbm_gbs
+            if clocks.get("sm_mhz"):
+                roof[kk]["frac_at_achieved_clock"] = roof[kk]["achieved"] / (ALU_LANES_PER_CLK * clocks["sm_mhz"] * 1e6 / 1e12)
+        dom = "query_kernel" if qk * 1.0 >= ik else "insert_kernel"
+        traffic = load_traffic(dom)
+        roofline = {"bound": "alu", "kernel": dom, "achieved": roof[dom]["achieved"], "peak": alu_peak,
+                    "unit": "Tiop/s", "frac": roof[dom]["frac"], "traffic": traffic,
+                    "peak_source": "derived: 148 SM x 64 int lanes/clk x %.0f MHz (%s sm_max_mhz), DESIGN.md §6" % (
+                        sm_max_mhz, peak_src),
+                    "hbm": {"achieved": roof[dom]["hbm_gbs_algorithmic"], "peak": hbm_gbs, "unit": "GB/s",
+                            "frac": roof[dom]["hbm_frac"], "peak_source": peak_src + " (MEASURED_PEAKS.json hbm_gbs)"}}
+        line = {
+            "metric": METRIC,
+            "value": value, "unit": "G k-mers/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u64", "data": "synthetic",
+            "config": {"workload": args.workload, "k": k, "m": p["m"], "s": p["s"], "H": p["H"],
+                       "filter_bits": num_bits, "insert_bases_per_rank": int(d_seq.numel()),
+                       "insert_kmers_per_rank": int(n_ins_kmers), "reads_per_batch": rb, "read_len": w.read_len,
+                       "read_batches": n_batches, "l2": "inputs larger than L2 (sequence %d MB, read batch %d MB, "
+                       "filter %d MiB); no flush" % (d_seq.numel() // 10**6, n_read_bases // 10**6, num_bits >> 23),
+                       "parallelism": "replicas x%d + OR all-reduce" % world if world > 1 else "single GPU"},
+            "insert_gkmers_s": ins_rate, "query_gkmers_s": q_rate,
+            "fpr": {"random_reads": fpr_random, "sampled_reads_hit_rate": hit_sampled,
+                    "bits_per_inserted_kmer": num_bits / max(1, n_ins_kmers)},
+            "clocks": clocks,
+            "e2e": {"value": e2e_kmers_all / e2e_s / 1e9, "unit": "G k-mers/s", "h2d_bytes_per_step": int(h2d),
+                    "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
+                    "api": "sbf_insert_seq_host + sbf_query_records_host (pinned host buffers)"},
+            "gpu_launches": int(launches),
+            "roofline": roofline, "rooflines": roof,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(args, w)
+        print(json.dumps(line))
+    sbf.sbf_destroy(h)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def load_traffic(kernel: str):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/traffic.json, written by hand from the .ncu-rep; null until a capture exists)."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        with open(p) as fh:
+            return json.load(fh).get(kernel)
+    except Exception:
+        return None
+
+
+def cpu_baseline(args, w):
+    import oracle
+    p = w.params
+    ins_bases = min(w.insert_bases.size, args.ref_insert_bases)
+    n_reads = min(max(w.n_reads, 1), args.ref_reads)
+    seq_s, reads_s, offs_s = make_oracle_sample(w, ins_bases, n_reads)
+    o = oracle.OracleSBF(p["k"], p["m"], p["s"], p["H"], p["num_bits"])
+    sample = "insert first %d bases of the %s sequence + query first %d reads x %d, filter %d bits" % (
+        ins_bases, args.workload, n_reads, w.read_len, o.num_bits)
+    a, b, ti, tq = oracle_sample_step(o, seq_s, reads_s, offs_s, False)
+    single = {"value": (a + b) / (ti + tq) / 1e9, "insert": a / ti / 1e9, "query": b / tq / 1e9}
+    a, b, ti, tq = oracle_sample_step(o, seq_s, reads_s, offs_s, True)
+    cores = oracle.num_threads()
+    return {"value": (a + b) / (ti + tq) / 1e9, "unit": "G k-mers/s", "cores": cores, "kind": "oracle",
+            "sample": sample, "insert_gkmers_s": a / ti / 1e9, "query_gkmers_s": b / tq / 1e9,
+            "single_thread": single}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3"])
+    ap.add_argument("--scale", type=float, default=1.0, help="shrink the workload (tests only)")
+    ap.add_argument("--read-batch", type=int, default=4_000_000, help="reads per query batch (one per step)")
+    ap.add_argument("--batches", type=int, default=4, help="distinct read batches rotated over the steps")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ref-scale", type=float, default=0.1, help="--impl reference: sequence generated at this scale")
+    ap.add_argument("--ref-insert-bases", type=int, default=10_000_000)
+    ap.add_argument("--ref-reads", type=int, default=50_000)
+    args = ap.parse_args()
+    if args.steps < 1 or args.warmup < 0:
+        raise SystemExit("need --steps >= 1, --warmup >= 0")
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

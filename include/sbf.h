@@ -138,11 +138,25 @@ const uint64_t *sbf_filter_device_ptr(const sbf_t *f);
  * The merge step of the replica scheme. */
 int sbf_or_bits_device(sbf_t *f, const uint64_t *d_src, uint64_t nbytes, void *stream);
 
+/* sbf_or_range_device — the same for a sub-range: filter[offset_bytes .. +nbytes) |= d_src[0 .. nbytes).
+ * offset_bytes and nbytes are multiples of 32 (whole shards), d_src is 16-byte aligned.  Lets the
+ * replica merge run window by window (paper_2606_24417_b200/replicas.py). */
+int sbf_or_range_device(sbf_t *f, uint64_t offset_bytes, const uint64_t *d_src, uint64_t nbytes, void *stream);
+
 /* Message for the last error on the calling thread ("" if none). */
 const char *sbf_last_error(void);
 
 /* Counts kernels launched by this library in this process (all handles); bench.py reports it. */
 uint64_t sbf_kernel_launches(void);
+
+/* sbf_set_timing — on != 0: every later device-facing insert/query call on this handle records CUDA
+ * events on the caller's stream around each kernel it enqueues (a few microseconds per call).
+ * sbf_get_timing — device time of the kernels of the LAST such call, in milliseconds:
+ *   ms3[0] = pack (+ record-end marking), ms3[1] = the fused insert or query kernel,
+ *   ms3[2] = the hit-count kernel (0 when none ran).  Waits for that call's last event.
+ * bench.py uses these for the per-kernel roofline figures. */
+int sbf_set_timing(sbf_t *f, int on);
+int sbf_get_timing(sbf_t *f, float *ms3);
 
 /* Diagnostics for tests: dump the internal 2-bit packed words / validity mask of the LAST batch
  * (device->host, synchronises).  n_words = ceil(bases/16); mask has one uint16 per word. */

@@ -48,8 +48,11 @@ ABI = {
     "sbf_import_bits": (_i32, [_p, _p, _u64]),
     "sbf_filter_device_ptr": (_p, [_p]),
     "sbf_or_bits_device": (_i32, [_p, _p, _u64, _p]),
+    "sbf_or_range_device": (_i32, [_p, _u64, _p, _u64, _p]),
     "sbf_last_error": (_cp, []),
     "sbf_kernel_launches": (_u64, []),
+    "sbf_set_timing": (_i32, [_p, _i32]),
+    "sbf_get_timing": (_i32, [_p, _p]),
     "sbf_debug_last_packed": (_i32, [_p, _p, _p, _u64]),
 }
 
@@ -192,6 +195,21 @@ def sbf_import_bits(h, bits: np.ndarray):
 
 def sbf_or_bits_device(h, d_src, nbytes: int, stream=None):
     _check(load_library().sbf_or_bits_device(h, _dptr(d_src), nbytes, _stream(stream)))
+
+
+def sbf_or_range_device(h, offset_bytes: int, d_src, nbytes: int, stream=None):
+    _check(load_library().sbf_or_range_device(h, offset_bytes, _dptr(d_src), nbytes, _stream(stream)))
+
+
+def sbf_set_timing(h, on: bool):
+    _check(load_library().sbf_set_timing(h, 1 if on else 0))
+
+
+def sbf_get_timing(h):
+    """(pack_ms, main_ms, count_ms) of the last device-facing call."""
+    ms = (ctypes.c_float * 3)()
+    _check(load_library().sbf_get_timing(h, ctypes.cast(ms, ctypes.c_void_p)))
+    return float(ms[0]), float(ms[1]), float(ms[2])
 
 
 def sbf_debug_last_packed(h, n_words: int):

@@ -99,6 +99,11 @@ struct sbf {
     bool l2_stream_valid;
     // host-facing staging (created on first use)
     HostRun *host;
+    // optional per-kernel timing (sbf_set_timing): events on the caller's stream around each kernel
+    bool timing;
+    cudaEvent_t tev[4]; // before pack, after pack, after main kernel, after count kernel
+    bool tev_count;     // the last call enqueued a count kernel
+    bool tev_valid;     // a timed call has completed its enqueue
 };
 
 namespace {
@@ -194,13 +199,29 @@ int run_main(sbf *f, uint64_t total, uint32_t *bitmap, cudaStream_t st)
     return SBF_OK;
 }
 
+int mark(sbf *f, int i, cudaStream_t st)
+{
+    if (!f->timing) return SBF_OK;
+    if (i == 0) { f->tev_count = false; f->tev_valid = false; }
+    if (i == 2) f->tev_valid = true;
+    if (i == 3) f->tev_count = true;
+    CK(cudaEventRecord(f->tev[i], st));
+    return SBF_OK;
+}
+
 int run_insert(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, cudaStream_t st)
 {
     if (total == 0) return SBF_OK;
     apply_l2_window(f, st);
-    int rc = run_pack(f, d_bases, d_offsets, n_rec, total, st);
+    int rc = mark(f, 0, st);
     if (rc) return rc;
-    return run_main<true>(f, total, nullptr, st);
+    rc = run_pack(f, d_bases, d_offsets, n_rec, total, st);
+    if (rc) return rc;
+    rc = mark(f, 1, st);
+    if (rc) return rc;
+    rc = run_main<true>(f, total, nullptr, st);
+    if (rc) return rc;
+    return mark(f, 2, st);
 }
 
 int run_query(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, uint32_t *d_bitmap,
@@ -208,9 +229,15 @@ int run_query(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n
 {
     if (total == 0) return SBF_OK;
     apply_l2_window(f, st);
-    int rc = run_pack(f, d_bases, d_offsets, n_rec, total, st);
+    int rc = mark(f, 0, st);
     if (rc) return rc;
-    return run_main<false>(f, total, d_bitmap, st);
+    rc = run_pack(f, d_bases, d_offsets, n_rec, total, st);
+    if (rc) return rc;
+    rc = mark(f, 1, st);
+    if (rc) return rc;
+    rc = run_main<false>(f, total, d_bitmap, st);
+    if (rc) return rc;
+    return mark(f, 2, st);
 }
 
 int run_count_records(const uint32_t *d_bitmap, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, uint32_t *d_counts,
@@ -294,6 +321,8 @@ void sbf_destroy(sbf_t *f)
     if (!f) return;
     cudaDeviceSynchronize();
     delete f->host;
+    for (int i = 0; i < 4; ++i)
+        if (f->tev[i]) cudaEventDestroy(f->tev[i]);
     if (f->packed) cudaFree(f->packed);
     if (f->gmask) cudaFree(f->gmask);
     if (f->filter) cudaFree(f->filter);
@@ -310,6 +339,31 @@ int sbf_reserve(sbf_t *f, uint64_t max_bases)
 {
     if (!f) return fail(SBF_ERR_INVALID_ARG, "sbf_reserve: NULL handle");
     return ensure_scratch(f, max_bases);
+}
+
+int sbf_set_timing(sbf_t *f, int on)
+{
+    if (!f) return fail(SBF_ERR_INVALID_ARG, "sbf_set_timing: NULL handle");
+    if (on)
+        for (int i = 0; i < 4; ++i)
+            if (!f->tev[i]) CK(cudaEventCreate(&f->tev[i]));
+    f->timing = on != 0;
+    f->tev_count = false;
+    f->tev_valid = false;
+    return SBF_OK;
+}
+
+int sbf_get_timing(sbf_t *f, float *ms3)
+{
+    if (!f || !ms3) return fail(SBF_ERR_INVALID_ARG, "sbf_get_timing: NULL argument");
+    if (!f->timing) return fail(SBF_ERR_INVALID_ARG, "sbf_get_timing: timing is off (sbf_set_timing)");
+    ms3[0] = ms3[1] = ms3[2] = 0.f;
+    if (!f->tev_valid) return fail(SBF_ERR_INVALID_ARG, "sbf_get_timing: no timed call yet");
+    CK(cudaEventSynchronize(f->tev[f->tev_count ? 3 : 2]));
+    CK(cudaEventElapsedTime(&ms3[0], f->tev[0], f->tev[1]));
+    CK(cudaEventElapsedTime(&ms3[1], f->tev[1], f->tev[2]));
+    if (f->tev_count) CK(cudaEventElapsedTime(&ms3[2], f->tev[2], f->tev[3]));
+    return SBF_OK;
 }
 
 int sbf_clear(sbf_t *f, void *stream)
@@ -347,6 +401,8 @@ int sbf_query_seq(sbf_t *f, const char *d_seq, uint64_t len, uint32_t *d_bitmap,
             count_total_kernel<<<blocks, 256, 0, st>>>(d_bitmap, nw, reinterpret_cast<unsigned long long *>(d_hits));
             CK(cudaGetLastError());
             g_launches++;
+            rc = mark(f, 3, st);
+            if (rc) return rc;
         }
     }
     return SBF_OK;
@@ -366,6 +422,8 @@ int sbf_query_records(sbf_t *f, const char *d_bases, const uint64_t *d_offsets, 
             CK(cudaMemsetAsync(d_hit_counts, 0, n_rec * sizeof(uint32_t), st));
         } else {
             rc = run_count_records(d_bitmap, d_offsets, n_rec, total_bases, d_hit_counts, st);
+            if (rc) return rc;
+            rc = mark(f, 3, st);
             if (rc) return rc;
         }
     }
@@ -397,6 +455,21 @@ int sbf_or_bits_device(sbf_t *f, const uint64_t *d_src, uint64_t nbytes, void *s
     uint64_t nw = f->num_shards * 4;
     unsigned blocks = (unsigned)((nw / 2 + 255) / 256 < 2368 ? (nw / 2 + 255) / 256 : 2368);
     or_words_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(f->filter, d_src, nw);
+    CK(cudaGetLastError());
+    g_launches++;
+    return SBF_OK;
+}
+
+int sbf_or_range_device(sbf_t *f, uint64_t offset_bytes, const uint64_t *d_src, uint64_t nbytes, void *stream)
+{
+    if (!f || !d_src) return fail(SBF_ERR_INVALID_ARG, "sbf_or_range_device: NULL argument");
+    if ((offset_bytes & 31) || (nbytes & 31) || offset_bytes + nbytes > f->num_shards * 32 ||
+        (reinterpret_cast<uintptr_t>(d_src) & 15))
+        return fail(SBF_ERR_INVALID_ARG, "sbf_or_range_device: range must be whole shards inside the filter, source 16-byte aligned");
+    uint64_t nw = nbytes / 8;
+    if (nw == 0) return SBF_OK;
+    unsigned blocks = (unsigned)((nw / 2 + 255) / 256 < 2368 ? (nw / 2 + 255) / 256 : 2368);
+    or_words_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(f->filter + offset_bytes / 8, d_src, nw);
     CK(cudaGetLastError());
     g_launches++;
     return SBF_OK;
