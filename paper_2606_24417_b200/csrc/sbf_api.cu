@@ -177,6 +177,7 @@ StreamParams make_params(sbf *f, uint64_t total, uint32_t *bitmap)
     p.shard_shift = 32 - f->P;
     p.bitmap = bitmap;
     p.n_bitmap_words = (total + 31) / 32;
+    p.ones = ~0ull;
     return p;
 }
 

@@ -17,6 +17,23 @@
 #include <type_traits>
 #include <utility>
 
+// ---- tuning switches (defaults = the measured best)
+#ifndef SBF_Q_LA
+#define SBF_Q_LA 4   // query: the minimizer runs this many positions ahead of the bit tests
+#endif
+#ifndef SBF_Q_PF
+#define SBF_Q_PF 1   // query: 0 no prefetch, 1 prefetch.global.L2, 2 prefetch.global.L1
+#endif
+#ifndef SBF_I_VAR
+#define SBF_I_VAR 0  // insert: accumulator scheme (see stream_kernel)
+#endif
+#ifndef SBF_MINB_I
+#define SBF_MINB_I 6 // insert: CTAs per SM the register budget is cut for (6 x 128 threads -> 80 registers)
+#endif
+#ifndef SBF_MINB_Q
+#define SBF_MINB_Q 8 // query: 8 x 128 threads -> 64 registers
+#endif
+
 namespace sbfk {
 
 // ---- pinned constants (A1, A2, A4, A6) -------------------------------------------------
@@ -39,6 +56,7 @@ struct StreamParams {
     int shard_shift;        // 32 - P
     uint32_t *bitmap;       // query: ceil(n_pos/32) words
     uint64_t n_bitmap_words;
+    uint64_t ones;          // all ones (opaque to the compiler)
 };
 
 struct NaiveParams {
@@ -175,36 +193,39 @@ __global__ void mark_ends_kernel(const uint64_t *__restrict__ offsets, uint64_t 
 #endif // SBF_DEFINE_AUX_KERNELS
 
 // =============================================================================================
-// Window access for stream_kernel.  W[0..2] hold 48 consecutive symbols (W[0] first, first symbol
+// Window access for stream_kernel.  W[0..3] hold 64 consecutive symbols (W[0] first, first symbol
 // in the top bits).  lmer<O,N>(W) = the N-mer starting O symbols into the window, as Sub() of the
 // paper's packed k-mer (first base most significant).  All shifts are immediates.
 // =============================================================================================
+constexpr int kWin = 4; // 32-bit words in the register window
+
 template <int Q, int NB>
-__device__ __forceinline__ uint32_t field96(const uint32_t (&W)[3])
+__device__ __forceinline__ uint32_t field_win(const uint32_t (&W)[kWin])
 {
-    static_assert(Q >= 0 && NB >= 1 && NB <= 32 && Q + NB <= 96, "field outside the 96-bit window");
+    // bits [Q, Q+NB) of the window, counted from the least significant bit of W[kWin-1]
+    static_assert(Q >= 0 && NB >= 1 && NB <= 32 && Q + NB <= 32 * kWin, "field outside the register window");
     constexpr int idx = Q / 32, sh = Q % 32;
-    uint32_t lo = W[2 - idx];
+    uint32_t lo = W[kWin - 1 - idx];
     uint32_t v;
     if constexpr (sh == 0) {
         v = lo;
     } else if constexpr (sh + NB <= 32) {
         v = lo >> sh;
     } else {
-        v = __funnelshift_r(lo, W[1 - idx], sh);
+        v = __funnelshift_r(lo, W[kWin - 2 - idx], sh);
     }
     if constexpr (NB < 32 && !(sh + NB == 32)) v &= (1u << NB) - 1u;
     return v;
 }
 
 template <int O, int N>
-__device__ __forceinline__ uint64_t lmer(const uint32_t (&W)[3])
+__device__ __forceinline__ uint64_t lmer(const uint32_t (&W)[kWin])
 {
-    constexpr int Q = 96 - 2 * O - 2 * N;
+    constexpr int Q = 32 * kWin - 2 * O - 2 * N;
     constexpr int nb = 2 * N;
-    uint32_t lo = field96<Q, (nb < 32 ? nb : 32)>(W);
+    uint32_t lo = field_win<Q, (nb < 32 ? nb : 32)>(W);
     uint32_t hi = 0;
-    if constexpr (nb > 32) hi = field96<Q + 32, nb - 32>(W);
+    if constexpr (nb > 32) hi = field_win<Q + 32, nb - 32>(W);
     return ((uint64_t)hi << 32) | lo;
 }
 
@@ -255,28 +276,48 @@ __device__ __forceinline__ void expand_masks(uint64_t h, uint64_t (&m)[NW])
 
 __host__ __device__ constexpr int ring_size(int z) { return z <= 1 ? 1 : z <= 2 ? 2 : z <= 4 ? 4 : z <= 8 ? 8 : 16; }
 
+// A2 with the shift clamped in hardware (shard_shift = 32 when there is one shard)
+__device__ __forceinline__ uint32_t sigma32(uint32_t key, int shard_shift)
+{
+    uint32_t t = (uint32_t)(((uint64_t)key * kGold64) >> 32);
+    return __funnelshift_rc(t, 0u, (uint32_t)shard_shift);
+}
+
+__device__ __forceinline__ void prefetch_shard(const uint64_t *p)
+{
+#if SBF_Q_PF == 2
+    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+#else
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+#endif
+}
+
 // =============================================================================================
 // a2-a6 fused.  One thread walks kChunk consecutive k-mer start positions p0 .. p0+kChunk-1 of the
-// batch, carrying in registers: the 48-symbol window, the sliding-minimum rings (a2), the one-hot
+// batch, carrying in registers: the 64-symbol window, the sliding-minimum rings (a2), the one-hot
 // masks of the last k-s s-mers, and
 //   insert: the OR of the current super-k-mer's masks (a5), flushed with one RED.OR.B64 per sector
-//           word when the minimizer key (hence the shard, A14) or validity changes;
-//   query : the current shard's 256 bits (a6), reloaded when the key changes; the k-mer's mask
+//           word when the shard (A14) or validity changes;
+//   query : the current shard's 256 bits (a6), reloaded when the shard changes; the k-mer's mask
 //           K = OR of its k-s+1 s-mer masks is tested with K & ~shard == 0 (Findere rule).
+//           The minimizer runs LA positions ahead of the tests so that the shard of an upcoming
+//           run can be prefetched long before its first test.
 // Each m-mer key and each s-mer hash is computed once per position (not once per k-mer as in
 // Alg. 1/2); the result bits are the same because OR/AND do not care about order or repetition.
 // =============================================================================================
 template <int K, int M, int S, int H, bool INSERT>
-__global__ void __launch_bounds__(kStreamTPB) stream_kernel(const StreamParams prm)
+__global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) stream_kernel(const StreamParams prm)
 {
     constexpr int WN = K - M + 1;
     constexpr int Z = K - S;
     constexpr int NW = H < 4 ? H : 4;
     constexpr int RZ = ring_size(Z);
     constexpr int L = K > 1 ? K - 1 : 1;
+    constexpr int LA = INSERT ? 0 : SBF_Q_LA;
     constexpr uint32_t maskL = (L >= 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
     static_assert(K >= 1 && K <= 32 && M >= 1 && M <= K && S >= 1 && S <= K, "bad k/m/s");
     static_assert(Z <= 16, "stream kernel supports k-s <= 16");
+    static_assert(LA >= 0 && LA <= 16 && (LA == 0 || 16 % LA == 0), "lookahead must divide 16");
 
     const uint64_t chunk = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint64_t p0 = chunk * kChunk;
@@ -284,9 +325,9 @@ __global__ void __launch_bounds__(kStreamTPB) stream_kernel(const StreamParams p
 
     const uint32_t *__restrict__ pw = prm.packed + (p0 >> 4);
     const uint16_t *__restrict__ gw = prm.gmask + (p0 >> 4);
-    uint32_t W[3] = {__ldg(pw), __ldg(pw + 1), __ldg(pw + 2)};
+    uint32_t W[kWin] = {__ldg(pw), __ldg(pw + 1), __ldg(pw + 2), __ldg(pw + 3)};
     uint32_t glo = (uint32_t)__ldg(gw) | ((uint32_t)__ldg(gw + 1) << 16);
-    uint32_t ghi = __ldg(gw + 2);
+    uint32_t ghi = (uint32_t)__ldg(gw + 2) | ((uint32_t)__ldg(gw + 3) << 16);
 
     SlidingMin<WN> smin;
 #pragma unroll
@@ -306,6 +347,18 @@ __global__ void __launch_bounds__(kStreamTPB) stream_kernel(const StreamParams p
         constexpr int I = decltype(ic)::value;
         expand_masks<H, NW>(f_hash(lmer<I, S>(W), S), Mh[I % RZ]);
     });
+    // query: shards of the first LA k-mers, prefetched
+    uint32_t kq[LA > 0 ? LA : 1];
+    uint32_t laPrev = 0xFFFFFFFFu;
+    (void)laPrev;
+    kq[0] = 0;
+    static_for<0, LA>([&](auto ec) {
+        constexpr int E = decltype(ec)::value + WN - 1;
+        const uint32_t sh = sigma32(smin.template push<E>(g_key(lmer<E, M>(W), M)), prm.shard_shift);
+        kq[decltype(ec)::value] = sh;
+        if (SBF_Q_PF != 0 && (decltype(ec)::value == 0 || sh != laPrev)) prefetch_shard(prm.filter + (uint64_t)sh * 4);
+        laPrev = sh;
+    });
 
     uint64_t acc[NW];   // insert: OR of the current run's masks
     uint64_t shard[4];  // query: the current shard's sector words
@@ -313,30 +366,84 @@ __global__ void __launch_bounds__(kStreamTPB) stream_kernel(const StreamParams p
     for (int q = 0; q < NW; ++q) acc[q] = 0;
 #pragma unroll
     for (int q = 0; q < 4; ++q) shard[q] = 0;
-    uint32_t prevKey = 0;
+    uint32_t prevShard = 0;
     bool prevInval = true; // insert: previous k-mer invalid; query: no shard loaded yet
     uint32_t res = 0;
 
     for (int b = 0; b < kChunk / 16; ++b) {
-        const uint32_t wnext = __ldg(pw + b + 3);
-        const uint32_t gnext = __ldg(gw + b + 3);
+        const uint32_t wnext = __ldg(pw + b + 4);
+        const uint32_t gnext = __ldg(gw + b + 4);
         uint32_t res16 = 0;
         static_for<0, 16>([&](auto jc) {
             constexpr int J = decltype(jc)::value;
-            // a2: key of the newest m-mer of k-mer p = p0+16b+J, then the window minimum
-            const uint32_t key = smin.template push<J + WN - 1>(g_key(lmer<J + WN - 1, M>(W), M));
-            // a4: the newest s-mer of that k-mer
+            // a2/a3: key of the newest m-mer of k-mer p+LA (p = p0+16b+J), its window minimum, its shard
+            const uint32_t shNew =
+                sigma32(smin.template push<J + LA + WN - 1>(g_key(lmer<J + LA + WN - 1, M>(W), M)), prm.shard_shift);
+            uint32_t sh = shNew;
+            if constexpr (LA > 0) {
+                if (SBF_Q_PF != 0 && shNew != laPrev) prefetch_shard(prm.filter + (uint64_t)shNew * 4);
+                laPrev = shNew;
+                sh = kq[J % LA];
+                kq[J % LA] = shNew;
+            }
+            // a4: the newest s-mer of k-mer p
             uint64_t Mn[NW];
             expand_masks<H, NW>(f_hash(lmer<J + Z, S>(W), S), Mn);
             // a1: validity of k-mer p
             const bool inval = (__funnelshift_r(glo, ghi, J) & maskL) != 0;
             if constexpr (INSERT) {
-                const bool brk = (key != prevKey) || (inval != prevInval);
+                const bool brk = (sh != prevShard) || (inval != prevInval);
+#if SBF_I_VAR == 3
+                // acc = s-mers [run start, p-1]; the run's last k-mer p-1 also owns the Z s-mers p .. p+Z-1
+                if (brk && !prevInval) { // a5: flush the finished run
+                    uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
+#pragma unroll
+                    for (int q = 0; q < NW; ++q) {
+                        uint64_t o = acc[q];
+#pragma unroll
+                        for (int i = 0; i < Z; ++i) o |= Mh[(J + i) % RZ][q];
+                        red_or_64(dst + q, o);
+                    }
+                }
+                {
+                    const uint64_t keep = brk ? 0ull : ~0ull;
+#pragma unroll
+                    for (int q = 0; q < NW; ++q) acc[q] = (acc[q] & keep) | (Z > 0 ? Mh[J % RZ][q] : Mn[q]);
+                }
+#elif SBF_I_VAR == 2
+                // branch-free: K = mask of k-mer p; acc restarts from K at a break
+                uint64_t Kq[NW];
+#pragma unroll
+                for (int q = 0; q < NW; ++q) {
+                    uint64_t r = Mn[q];
+#pragma unroll
+                    for (int i = 0; i < Z; ++i) r |= Mh[(J + i) % RZ][q];
+                    Kq[q] = r;
+                }
+                if (brk && !prevInval) {
+                    uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
+#pragma unroll
+                    for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
+                }
+                {
+                    const uint64_t keep = brk ? 0ull : ~0ull;
+#pragma unroll
+                    for (int q = 0; q < NW; ++q) acc[q] = (acc[q] & keep) | Kq[q];
+                }
+#else
                 if (brk) {
                     if (!prevInval) { // a5: flush the finished run
-                        uint64_t *dst = prm.filter + sigma_shard(prevKey, prm.shard_shift) * 4;
+                        uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
+#if SBF_I_VAR == 1
+                        uint64_t o[NW];
+#pragma unroll
+                        for (int q = 0; q < NW; ++q) o[q] = acc[q] & prm.ones;
+#pragma unroll
+                        for (int q = 0; q < NW; ++q) red_or_64(dst + q, o[q]);
+#else
 #pragma unroll
                         for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
+#endif
                     }
 #pragma unroll
                     for (int q = 0; q < NW; ++q) { // restart with the k-s s-mers shared with the previous k-mers
@@ -348,31 +455,32 @@ __global__ void __launch_bounds__(kStreamTPB) stream_kernel(const StreamParams p
                 }
 #pragma unroll
                 for (int q = 0; q < NW; ++q) acc[q] |= Mn[q];
-                prevKey = key;
+#endif
+                prevShard = sh;
                 prevInval = inval;
             } else {
-                const bool need = !inval && (prevInval || key != prevKey);
+                const bool need = !inval && (prevInval || sh != prevShard);
                 if (need) { // a6: fetch the shard of the new run
-                    ld_shard_256(prm.filter + sigma_shard(key, prm.shard_shift) * 4, shard);
-                    prevKey = key;
+                    ld_shard_256(prm.filter + (uint64_t)sh * 4, shard);
+                    prevShard = sh;
                     prevInval = false;
                 }
                 uint64_t miss = 0;
 #pragma unroll
                 for (int q = 0; q < NW; ++q) {
-                    uint64_t kq = Mn[q];
+                    uint64_t kq_ = Mn[q];
 #pragma unroll
-                    for (int i = 0; i < Z; ++i) kq |= Mh[(J + i) % RZ][q];
-                    miss |= kq & ~shard[q];
+                    for (int i = 0; i < Z; ++i) kq_ |= Mh[(J + i) % RZ][q];
+                    miss |= kq_ & ~shard[q];
                 }
                 if (!inval && miss == 0) res16 |= 1u << J;
             }
 #pragma unroll
             for (int q = 0; q < NW; ++q) Mh[(J + Z) % RZ][q] = Mn[q];
         });
-        W[0] = W[1]; W[1] = W[2]; W[2] = wnext;
+        W[0] = W[1]; W[1] = W[2]; W[2] = W[3]; W[3] = wnext;
         glo = (glo >> 16) | (ghi << 16);
-        ghi = gnext;
+        ghi = (ghi >> 16) | (gnext << 16);
         if constexpr (!INSERT) {
             res = (res >> 16) | (res16 << 16);
             if (b & 1) {
@@ -383,9 +491,17 @@ __global__ void __launch_bounds__(kStreamTPB) stream_kernel(const StreamParams p
     }
     if constexpr (INSERT) {
         if (!prevInval) {
-            uint64_t *dst = prm.filter + sigma_shard(prevKey, prm.shard_shift) * 4;
+            uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
 #pragma unroll
-            for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
+            for (int q = 0; q < NW; ++q) {
+                uint64_t o = acc[q];
+#if SBF_I_VAR == 3
+                // after the loop the ring holds s-mers pEnd .. pEnd+Z-1 at slots (i % RZ), pEnd = 0 mod 16
+#pragma unroll
+                for (int i = 0; i < Z; ++i) o |= Mh[i % RZ][q];
+#endif
+                red_or_64(dst + q, o);
+            }
         }
     }
 }
