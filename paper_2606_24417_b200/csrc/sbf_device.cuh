@@ -19,10 +19,10 @@
 
 // ---- tuning switches (defaults = the measured best)
 #ifndef SBF_Q_LA
-#define SBF_Q_LA 4   // query: the minimizer runs this many positions ahead of the bit tests
+#define SBF_Q_LA 3   // query: the minimizer runs this many positions ahead of the bit tests
 #endif
 #ifndef SBF_Q_PF
-#define SBF_Q_PF 1   // query: 0 no prefetch, 1 prefetch.global.L2, 2 prefetch.global.L1
+#define SBF_Q_PF 3   // query: 0 no prefetch, 1 prefetch.global.L2, 2 prefetch.global.L1, 3 cp.async staging in shared memory
 #endif
 #ifndef SBF_I_VAR
 #define SBF_I_VAR 0  // insert: accumulator scheme (see stream_kernel)
@@ -31,7 +31,7 @@
 #define SBF_MINB_I 6 // insert: CTAs per SM the register budget is cut for (6 x 128 threads -> 80 registers)
 #endif
 #ifndef SBF_MINB_Q
-#define SBF_MINB_Q 8 // query: 8 x 128 threads -> 64 registers
+#define SBF_MINB_Q 5 // query: 5 x 128 threads -> 96 registers
 #endif
 
 namespace sbfk {
@@ -283,6 +283,18 @@ __device__ __forceinline__ uint32_t sigma32(uint32_t key, int shard_shift)
     return __funnelshift_rc(t, 0u, (uint32_t)shard_shift);
 }
 
+// query staging through shared memory (SBF_Q_PF == 3): the 32 bytes of a shard travel global -> shared with two
+// 16-byte cp.async (LDGSTS, no register in between) LA positions before the run's first test reads them back.
+__device__ __forceinline__ void cp_async_shard(uint4 *smem_lo, uint4 *smem_hi, const uint64_t *g)
+{
+    uint32_t a = (uint32_t)__cvta_generic_to_shared(smem_lo), b = (uint32_t)__cvta_generic_to_shared(smem_hi);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(a), "l"(g) : "memory");
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(b), "l"(g + 2) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 __device__ __forceinline__ void prefetch_shard(const uint64_t *p)
 {
 #if SBF_Q_PF == 2
@@ -317,7 +329,7 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
     constexpr uint32_t maskL = (L >= 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
     static_assert(K >= 1 && K <= 32 && M >= 1 && M <= K && S >= 1 && S <= K, "bad k/m/s");
     static_assert(Z <= 16, "stream kernel supports k-s <= 16");
-    static_assert(LA >= 0 && LA <= 16 && (LA == 0 || 16 % LA == 0), "lookahead must divide 16");
+    static_assert(LA >= 0 && LA <= 16 && (LA == 0 || SBF_Q_PF == 3 || 16 % LA == 0), "lookahead must divide 16");
 
     const uint64_t chunk = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint64_t p0 = chunk * kChunk;
@@ -347,16 +359,33 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
         constexpr int I = decltype(ic)::value;
         expand_masks<H, NW>(f_hash(lmer<I, S>(W), S), Mh[I % RZ]);
     });
-    // query: shards of the first LA k-mers, prefetched
+    // query: shards of the first LA k-mers, prefetched (PF 1/2) or staged in shared memory (PF 3)
+    constexpr bool STAGE = !INSERT && SBF_Q_PF == 3;
+    constexpr int NS = LA + 1; // staging slots per thread: k-mer q uses slot q mod NS
+    static_assert(!STAGE || (LA >= 1 && 16 % NS == 0), "staging needs LA in {1,3,7,15}");
+    __shared__ uint4 stage[STAGE ? NS * 2 * kStreamTPB : 1];
     uint32_t kq[LA > 0 ? LA : 1];
-    uint32_t laPrev = 0xFFFFFFFFu;
-    (void)laPrev;
+    uint32_t laPrev = 0xFFFFFFFFu, sb = 0;
+    bool laInv = true;
+    (void)laPrev; (void)sb; (void)laInv; (void)stage;
     kq[0] = 0;
     static_for<0, LA>([&](auto ec) {
-        constexpr int E = decltype(ec)::value + WN - 1;
+        constexpr int Q = decltype(ec)::value;
+        constexpr int E = Q + WN - 1;
         const uint32_t sh = sigma32(smin.template push<E>(g_key(lmer<E, M>(W), M)), prm.shard_shift);
-        kq[decltype(ec)::value] = sh;
-        if (SBF_Q_PF != 0 && (decltype(ec)::value == 0 || sh != laPrev)) prefetch_shard(prm.filter + (uint64_t)sh * 4);
+        if constexpr (STAGE) {
+            const bool invN = (__funnelshift_r(glo, ghi, Q) & maskL) != 0;
+            const bool start = !invN && (laInv || sh != laPrev);
+            if (start)
+                cp_async_shard(&stage[((Q % NS) * 2) * kStreamTPB + threadIdx.x], &stage[((Q % NS) * 2 + 1) * kStreamTPB + threadIdx.x],
+                               prm.filter + (uint64_t)sh * 4);
+            cp_async_commit();
+            sb |= (start ? 1u : 0u) << Q;
+            laInv = invN;
+        } else {
+            kq[Q] = sh;
+            if (SBF_Q_PF != 0 && (Q == 0 || sh != laPrev)) prefetch_shard(prm.filter + (uint64_t)sh * 4);
+        }
         laPrev = sh;
     });
 
@@ -380,7 +409,17 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
             const uint32_t shNew =
                 sigma32(smin.template push<J + LA + WN - 1>(g_key(lmer<J + LA + WN - 1, M>(W), M)), prm.shard_shift);
             uint32_t sh = shNew;
-            if constexpr (LA > 0) {
+            if constexpr (STAGE) {
+                const bool invN = (__funnelshift_r(glo, ghi, J + LA) & maskL) != 0;
+                const bool start = !invN && (laInv || shNew != laPrev);
+                if (start)
+                    cp_async_shard(&stage[(((J + LA) % NS) * 2) * kStreamTPB + threadIdx.x],
+                                   &stage[(((J + LA) % NS) * 2 + 1) * kStreamTPB + threadIdx.x], prm.filter + (uint64_t)shNew * 4);
+                cp_async_commit();
+                sb |= (start ? 1u : 0u) << LA;
+                laInv = invN;
+                laPrev = shNew;
+            } else if constexpr (LA > 0) {
                 if (SBF_Q_PF != 0 && shNew != laPrev) prefetch_shard(prm.filter + (uint64_t)shNew * 4);
                 laPrev = shNew;
                 sh = kq[J % LA];
@@ -459,11 +498,22 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
                 prevShard = sh;
                 prevInval = inval;
             } else {
-                const bool need = !inval && (prevInval || sh != prevShard);
-                if (need) { // a6: fetch the shard of the new run
-                    ld_shard_256(prm.filter + (uint64_t)sh * 4, shard);
-                    prevShard = sh;
-                    prevInval = false;
+                if constexpr (STAGE) {
+                    if (sb & 1u) { // a6: the run starting here: its shard was staged LA positions ago
+                        cp_async_wait<LA>();
+                        const uint4 lo = stage[((J % NS) * 2) * kStreamTPB + threadIdx.x];
+                        const uint4 hi = stage[((J % NS) * 2 + 1) * kStreamTPB + threadIdx.x];
+                        shard[0] = ((uint64_t)lo.y << 32) | lo.x; shard[1] = ((uint64_t)lo.w << 32) | lo.z;
+                        shard[2] = ((uint64_t)hi.y << 32) | hi.x; shard[3] = ((uint64_t)hi.w << 32) | hi.z;
+                    }
+                    sb >>= 1;
+                } else {
+                    const bool need = !inval && (prevInval || sh != prevShard);
+                    if (need) { // a6: fetch the shard of the new run
+                        ld_shard_256(prm.filter + (uint64_t)sh * 4, shard);
+                        prevShard = sh;
+                        prevInval = false;
+                    }
                 }
                 uint64_t miss = 0;
 #pragma unroll
