@@ -27,6 +27,9 @@
 #ifndef SBF_I_VAR
 #define SBF_I_VAR 0  // insert: accumulator scheme (see stream_kernel)
 #endif
+#ifndef SBF_ONEHOT
+#define SBF_ONEHOT 0  // one-hot masks by plain shifts (0) or through a float exponent + F2I (1; measured: no gain)
+#endif
 #ifndef SBF_MINB_I
 #define SBF_MINB_I 6 // insert: CTAs per SM the register budget is cut for (6 x 128 threads -> 80 registers)
 #endif
@@ -93,6 +96,15 @@ __device__ __forceinline__ uint64_t f_hash(uint64_t x, int s)
 {
     x ^= kSeedS & low_mask64(2 * s);
     uint64_t h = (x ^ (x >> 28)) * kMultF;
+    return h ^ (h >> 32);
+}
+// the same value with the seed folded: ((x^sd) ^ ((x^sd)>>28)) = x ^ (x>>28) ^ (sd ^ (sd>>28))  (one LOP3 per half)
+template <int S>
+__device__ __forceinline__ uint64_t f_hash_c(uint64_t x)
+{
+    constexpr uint64_t sd = kSeedS & low_mask64(2 * S);
+    constexpr uint64_t c = sd ^ (sd >> 28);
+    uint64_t h = (x ^ (x >> 28) ^ c) * kMultF;
     return h ^ (h >> 32);
 }
 // A5 / A6: bit position of hash index i inside sector word i mod 4
@@ -260,7 +272,31 @@ struct SlidingMin {
     }
 };
 
-// One-hot sector masks of one s-mer hash: hash index i -> word i mod 4, bit B(h,i) (A5)
+// One-hot sector masks of one s-mer hash: hash index i -> word i mod 4, bit B(h,i) (A5).
+// SBF_ONEHOT == 1 builds 1 << b off the saturated ALU pipe: the 6 bits of b are moved into the exponent
+// field of a float (2^(b+1), one LOP3), halved on the FMA pipe and converted with one F2I.U64 (XU pipe);
+// every step is exact.  SBF_ONEHOT == 0 is the plain shift form (two SHF per bit on the ALU pipe).
+template <int OFF>
+__device__ __forceinline__ uint64_t onehot_at(uint64_t h)
+{
+#if SBF_ONEHOT == 1
+    constexpr int o = OFF % 32;
+    if constexpr (o + 6 <= 32) {
+        const uint32_t half = OFF < 32 ? (uint32_t)h : (uint32_t)(h >> 32);
+        uint32_t t;
+        if constexpr (o <= 23) t = half << (23 - o);
+        else t = half >> (o - 23);
+        const float f = __uint_as_float((t & 0x1F800000u) | 0x40000000u) * 0.5f; // 2^b
+        return __float2ull_rz(f);
+    } else {
+        const uint32_t b = (uint32_t)(h >> OFF) & 63u;
+        return __float2ull_rz(__uint_as_float((b << 23) | 0x40000000u) * 0.5f);
+    }
+#else
+    return 1ull << ((h >> OFF) & 63);
+#endif
+}
+
 template <int H, int NW>
 __device__ __forceinline__ void expand_masks(uint64_t h, uint64_t (&m)[NW])
 {
@@ -270,7 +306,7 @@ __device__ __forceinline__ void expand_masks(uint64_t h, uint64_t (&m)[NW])
     for (int q = 0; q < NW; ++q) m[q] = 0;
     static_for<0, H>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        m[i & 3] |= 1ull << ((h >> (i * Wd)) & 63);
+        m[i & 3] |= onehot_at<i * Wd>(h);
     });
 }
 
@@ -357,15 +393,24 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
     });
     static_for<0, Z>([&](auto ic) {
         constexpr int I = decltype(ic)::value;
-        expand_masks<H, NW>(f_hash(lmer<I, S>(W), S), Mh[I % RZ]);
+        expand_masks<H, NW>(f_hash_c<S>(lmer<I, S>(W)), Mh[I % RZ]);
     });
+    uint64_t PB[NW], PC[NW]; // query, Z == 3: ORs of adjacent mask pairs (see the test below)
+#pragma unroll
+    for (int q = 0; q < NW; ++q) {
+        PB[q] = Mh[0][q] | Mh[1 % RZ][q];
+        PC[q] = Mh[1 % RZ][q] | Mh[2 % RZ][q];
+    }
     // query: shards of the first LA k-mers, prefetched (PF 1/2) or staged in shared memory (PF 3)
     constexpr bool STAGE = !INSERT && SBF_Q_PF == 3;
     constexpr int NS = LA + 1; // staging slots per thread: k-mer q uses slot q mod NS
     static_assert(!STAGE || (LA >= 1 && 16 % NS == 0), "staging needs LA in {1,3,7,15}");
     __shared__ uint4 stage[STAGE ? NS * 2 * kStreamTPB : 1];
     uint32_t kq[LA > 0 ? LA : 1];
-    uint32_t laPrev = 0xFFFFFFFFu, sb = 0;
+    uint32_t laPrev = 0xFFFFFFFFu;
+    bool sb[NS]; // sb[q mod NS]: a run starts at k-mer q (its shard is in staging slot q mod NS)
+#pragma unroll
+    for (int i = 0; i < NS; ++i) sb[i] = false;
     bool laInv = true;
     (void)laPrev; (void)sb; (void)laInv; (void)stage;
     kq[0] = 0;
@@ -380,7 +425,7 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
                 cp_async_shard(&stage[((Q % NS) * 2) * kStreamTPB + threadIdx.x], &stage[((Q % NS) * 2 + 1) * kStreamTPB + threadIdx.x],
                                prm.filter + (uint64_t)sh * 4);
             cp_async_commit();
-            sb |= (start ? 1u : 0u) << Q;
+            sb[Q % NS] = start;
             laInv = invN;
         } else {
             kq[Q] = sh;
@@ -409,6 +454,7 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
             const uint32_t shNew =
                 sigma32(smin.template push<J + LA + WN - 1>(g_key(lmer<J + LA + WN - 1, M>(W), M)), prm.shard_shift);
             uint32_t sh = shNew;
+            (void)sh;
             if constexpr (STAGE) {
                 const bool invN = (__funnelshift_r(glo, ghi, J + LA) & maskL) != 0;
                 const bool start = !invN && (laInv || shNew != laPrev);
@@ -416,7 +462,7 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
                     cp_async_shard(&stage[(((J + LA) % NS) * 2) * kStreamTPB + threadIdx.x],
                                    &stage[(((J + LA) % NS) * 2 + 1) * kStreamTPB + threadIdx.x], prm.filter + (uint64_t)shNew * 4);
                 cp_async_commit();
-                sb |= (start ? 1u : 0u) << LA;
+                sb[(J + LA) % NS] = start;
                 laInv = invN;
                 laPrev = shNew;
             } else if constexpr (LA > 0) {
@@ -427,7 +473,7 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
             }
             // a4: the newest s-mer of k-mer p
             uint64_t Mn[NW];
-            expand_masks<H, NW>(f_hash(lmer<J + Z, S>(W), S), Mn);
+            expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
             // a1: validity of k-mer p
             const bool inval = (__funnelshift_r(glo, ghi, J) & maskL) != 0;
             if constexpr (INSERT) {
@@ -499,14 +545,13 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
                 prevInval = inval;
             } else {
                 if constexpr (STAGE) {
-                    if (sb & 1u) { // a6: the run starting here: its shard was staged LA positions ago
+                    if (sb[J % NS]) { // a6: the run starting here: its shard was staged LA positions ago
                         cp_async_wait<LA>();
                         const uint4 lo = stage[((J % NS) * 2) * kStreamTPB + threadIdx.x];
                         const uint4 hi = stage[((J % NS) * 2 + 1) * kStreamTPB + threadIdx.x];
                         shard[0] = ((uint64_t)lo.y << 32) | lo.x; shard[1] = ((uint64_t)lo.w << 32) | lo.z;
                         shard[2] = ((uint64_t)hi.y << 32) | hi.x; shard[3] = ((uint64_t)hi.w << 32) | hi.z;
                     }
-                    sb >>= 1;
                 } else {
                     const bool need = !inval && (prevInval || sh != prevShard);
                     if (need) { // a6: fetch the shard of the new run
@@ -516,12 +561,28 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
                     }
                 }
                 uint64_t miss = 0;
+                if constexpr (Z == 3) {
+                    // pair ORs: PB = M[t-2]|M[t-3], PC = M[t-1]|M[t-2]; K = (Mn | M[t-1]) | PB
+                    uint64_t mq[NW];
 #pragma unroll
-                for (int q = 0; q < NW; ++q) {
-                    uint64_t kq_ = Mn[q];
+                    for (int q = 0; q < NW; ++q) {
+                        const uint64_t cn = Mn[q] | Mh[(J + 2) % RZ][q];
+                        mq[q] = (cn | PB[q]) & ~shard[q];
+                        PB[q] = PC[q];
+                        PC[q] = cn;
+                    }
+                    if constexpr (NW == 4) miss = (mq[0] | mq[1] | mq[2]) | mq[3];
+                    else
 #pragma unroll
-                    for (int i = 0; i < Z; ++i) kq_ |= Mh[(J + i) % RZ][q];
-                    miss |= kq_ & ~shard[q];
+                        for (int q = 0; q < NW; ++q) miss |= mq[q];
+                } else {
+#pragma unroll
+                    for (int q = 0; q < NW; ++q) {
+                        uint64_t kq_ = Mn[q];
+#pragma unroll
+                        for (int i = 0; i < Z; ++i) kq_ |= Mh[(J + i) % RZ][q];
+                        miss |= kq_ & ~shard[q];
+                    }
                 }
                 if (!inval && miss == 0) res16 |= 1u << J;
             }
