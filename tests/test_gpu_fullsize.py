@@ -1,0 +1,129 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times
+(one sbf_insert_seq over the whole sequence, one sbf_query_records per 4e6-read batch, 2^32-bit filter).
+The oracle's OpenMP driver (pinned equal to the single-threaded definition by P6) makes the full
+comparison affordable: every filter byte, every bitmap word and every hit count, tolerance 0."""
+import numpy as np
+import pytest
+
+import oracle
+import seqgen
+import paper_2606_24417_b200 as sbf
+
+torch = pytest.importorskip("torch")
+pytestmark = [pytest.mark.gpu, pytest.mark.slow]
+
+DEFAULT = dict(k=31, m=16, s=28, H=4)
+
+
+def _dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _first_diff(got, want, what):
+    if np.array_equal(got, want):
+        return
+    bad = np.flatnonzero(got != want)
+    raise AssertionError("%s differs in %d of %d elements, first at %d: got %r want %r" %
+                         (what, bad.size, got.size, bad[0], got[bad[0]], want[bad[0]]))
+
+
+def test_config3_full_size_filter_bitmap_counts():
+    w = seqgen.config3()                       # 250 Mbp, N runs, 2^32-bit filter
+    nb = w.params["num_bits"]
+    n_reads = 4_000_000                        # bench.py's batch
+    reads = w.read_batch(0, n_reads)
+    offs = seqgen.fixed_offsets(n_reads, w.read_len)
+    o = oracle.OracleSBF(num_bits=nb, **DEFAULT)
+    n_ins = o.insert_records(w.insert_bases, threads=True)
+    assert 240_000_000 < n_ins < 250_000_000
+    with sbf.SuperBloomFilter(num_bits=nb, **DEFAULT) as f:
+        assert f.specialized and f.num_shards == o.num_shards == 1 << 24
+        d_seq = _dev(w.insert_bases)
+        f.insert_seq(d_seq)
+        torch.cuda.synchronize()
+        _first_diff(f.export_bits(), o.export_bits(), "filter bytes")
+        d_reads, d_offs = _dev(reads), _dev(offs.view(np.int64))
+        bm = torch.full(((reads.size + 31) // 32,), -1, dtype=torch.int32, device="cuda")
+        hc = torch.full((n_reads,), -1, dtype=torch.int32, device="cuda")
+        f.query_records(d_reads, d_offs, bm, hc)
+        torch.cuda.synchronize()
+        wbm, wc, n_q = o.query_records(reads, offs, threads=True)
+        _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "bitmap words")
+        _first_diff(hc.cpu().numpy().view(np.uint32), wc, "hit counts")
+        # properties that hold at any size: error-free k-mers of sampled reads are all present
+        per = w.read_len - DEFAULT["k"] + 1
+        sampled_hits = wc[0::2].astype(np.int64).sum()
+        assert sampled_hits > 0.6 * (n_reads // 2) * per
+        # FPR on the uniform reads stays small at 17 bits per k-mer
+        assert wc[1::2].astype(np.int64).sum() < 1e-3 * (n_reads // 2) * per
+    o.close()
+
+
+def test_config4_shape_4gib_filter_multi_record():
+    """2^35-bit filter (P = 27 shards, 64-bit byte offsets) with a 24-record insert at 1/25 scale."""
+    w = seqgen.config4(scale=0.04, n_reads=200_000)   # 124 Mbp in 24 records
+    nb = 1 << 35
+    o = oracle.OracleSBF(num_bits=nb, **DEFAULT)
+    o.insert_records(w.insert_bases, w.insert_offsets, threads=True)
+    with sbf.SuperBloomFilter(num_bits=nb, **DEFAULT) as f:
+        assert f.num_shards == 1 << 27
+        f.insert_records(_dev(w.insert_bases), _dev(w.insert_offsets.view(np.int64)))
+        torch.cuda.synchronize()
+        _first_diff(f.export_bits(), o.export_bits(), "filter bytes")
+        reads = w.read_batch(0, 200_000)
+        offs = seqgen.fixed_offsets(200_000, w.read_len)
+        bm = torch.full(((reads.size + 31) // 32,), -1, dtype=torch.int32, device="cuda")
+        hc = torch.full((200_000,), -1, dtype=torch.int32, device="cuda")
+        f.query_records(_dev(reads), _dev(offs.view(np.int64)), bm, hc)
+        torch.cuda.synchronize()
+        wbm, wc, _ = o.query_records(reads, offs, threads=True)
+        _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "bitmap words")
+        _first_diff(hc.cpu().numpy().view(np.uint32), wc, "hit counts")
+    o.close()
+
+
+def test_config2_full_size():
+    w = seqgen.config2()
+    distinct = seqgen.count_distinct_windows(w.insert_bases, DEFAULT["k"])  # exact (plain string set)
+    assert 4_500_000 < distinct < 5_000_000
+    nb = 16 * distinct
+    reads = w.read_batch(0, w.n_reads)
+    offs = seqgen.fixed_offsets(w.n_reads, w.read_len)
+    o = oracle.OracleSBF(num_bits=nb, **DEFAULT)
+    o.insert_records(w.insert_bases, threads=True)
+    with sbf.SuperBloomFilter(num_bits=nb, **DEFAULT) as f:
+        assert f.num_shards == o.num_shards == 1 << 19
+        f.insert_seq(_dev(w.insert_bases))
+        torch.cuda.synchronize()
+        _first_diff(f.export_bits(), o.export_bits(), "filter bytes")
+        bm = torch.full(((reads.size + 31) // 32,), -1, dtype=torch.int32, device="cuda")
+        hc = torch.full((w.n_reads,), -1, dtype=torch.int32, device="cuda")
+        f.query_records(_dev(reads), _dev(offs.view(np.int64)), bm, hc)
+        torch.cuda.synchronize()
+        wbm, wc, _ = o.query_records(reads, offs, threads=True)
+        _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "bitmap words")
+        _first_diff(hc.cpu().numpy().view(np.uint32), wc, "hit counts")
+    o.close()
+
+
+def test_timing_abi_reports_kernel_times():
+    seq = seqgen.uniform(5, 2_000_000)
+    with sbf.SuperBloomFilter(num_bits=1 << 26, **DEFAULT) as f:
+        with pytest.raises(sbf.SBFError):
+            sbf.sbf_get_timing(f.handle)          # timing is off
+        sbf.sbf_set_timing(f.handle, True)
+        with pytest.raises(sbf.SBFError):
+            sbf.sbf_get_timing(f.handle)          # no timed call yet
+        d = _dev(seq)
+        f.insert_seq(d)
+        pack_ms, main_ms, count_ms = sbf.sbf_get_timing(f.handle)
+        assert pack_ms > 0 and main_ms > 0 and count_ms == 0
+        bm = torch.empty((seq.size + 31) // 32, dtype=torch.int32, device="cuda")
+        hits = torch.zeros(1, dtype=torch.int64, device="cuda")
+        f.query_seq(d, bm, hits)
+        pack_ms, main_ms, count_ms = sbf.sbf_get_timing(f.handle)
+        assert pack_ms > 0 and main_ms > 0 and count_ms > 0
+        assert int(hits.item()) == seq.size - DEFAULT["k"] + 1
+        n0 = sbf.sbf_kernel_launches()
+        f.insert_seq(d)
+        assert sbf.sbf_kernel_launches() - n0 == 2   # pack + fused insert kernel
