@@ -152,7 +152,7 @@ int run_pack(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_
     if (rc) return rc;
     uint64_t nw = words_for(total);
     f->last_words = nw;
-    unsigned blocks = (unsigned)((nw + 255) / 256);
+    unsigned blocks = (unsigned)(((nw + 1) / 2 + 255) / 256);
     int aligned = ((reinterpret_cast<uintptr_t>(d_bases) & 15) == 0) ? 1 : 0;
     pack_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<const uint8_t *>(d_bases), total, f->packed, f->gmask, nw, f->k,
                                         aligned);

@@ -127,7 +127,7 @@ __device__ __forceinline__ void red_or_64(uint64_t *p, uint64_t v)
 }
 
 // =============================================================================================
-// a1: pack.  Thread i produces packed word i and mask word i from symbols [16i, 16i+16).
+// a1: pack.  Thread i produces packed words 2i, 2i+1 and their mask words from symbols [32i, 32i+32).
 //   code: A=0 C=1 G=2 T=3 (either case, A9); anything else is invalid (code bits arbitrary).
 //   B[j] = symbol j invalid or j >= len.   G[j] = B[j] | B[j+1] (k >= 2), = B[j] (k == 1).
 //   A k-mer starting at p is valid iff G[p .. p+max(k-1,1)-1] are all 0 once mark_ends_kernel
@@ -136,9 +136,14 @@ __device__ __forceinline__ void red_or_64(uint64_t *p, uint64_t v)
 __device__ __forceinline__ uint32_t pack4(uint32_t v, uint32_t &inv4)
 {
     // four ASCII bytes (first symbol in the low byte) -> 8 bits, first symbol in the top 2 bits
-    uint32_t u = v & 0xDFDFDFDFu;
-    uint32_t ok = __vcmpeq4(u, 0x41414141u) | __vcmpeq4(u, 0x43434343u) | __vcmpeq4(u, 0x47474747u) |
-                  __vcmpeq4(u, 0x54545454u);
+    // validity as a boolean function of the bit planes (bit 0 of every byte of v >> j is bit j of that symbol;
+    // bit 5, the case bit, is ignored): A 0x41, C 0x43, G 0x47, T 0x54 <=> !b7 & b6 & !b3 &
+    // (b4 ? (b2 & !b1 & !b0) : (b0 & (b1 | !b2))).  Six shifts and five LOP3 for four symbols.
+    const uint32_t s1 = v >> 1, s2 = v >> 2, s3 = v >> 3, s4 = v >> 4, s6 = v >> 6, s7 = v >> 7;
+    const uint32_t t1 = v & (s1 | ~s2);
+    const uint32_t t2 = s2 & ~s1 & ~v;
+    const uint32_t t3 = (s4 & t2) | (~s4 & t1);
+    const uint32_t ok = t3 & (~s7 & s6 & ~s3);
     uint32_t x = (v >> 1) & 0x03030303u;
     uint32_t c = x ^ ((x >> 1) & 0x01010101u);
     inv4 = ((~ok & 0x01010101u) * 0x10204080u) >> 28; // bit j = symbol j invalid
@@ -149,45 +154,51 @@ __device__ __forceinline__ uint32_t pack4(uint32_t v, uint32_t &inv4)
 __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ seq, uint64_t len, uint32_t *__restrict__ packed,
                                                    uint16_t *__restrict__ gmask, uint64_t n_words_total, int k, int aligned16)
 {
-    uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    uint64_t b0 = i * 16;
-    uint32_t v[4];
-    if (aligned16 && b0 + 16 <= len) {
-        uint4 q = __ldg(reinterpret_cast<const uint4 *>(seq + b0));
-        v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+    // thread i: symbols [32i, 32i+32) -> packed words 2i, 2i+1 (one 8-byte store) and their two mask words (one 4-byte store)
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint64_t b0 = i * 32;
+    uint32_t v[8];
+    if (aligned16 && b0 + 32 <= len) {
+        const uint4 q0 = __ldg(reinterpret_cast<const uint4 *>(seq + b0));
+        const uint4 q1 = __ldg(reinterpret_cast<const uint4 *>(seq + b0 + 16));
+        v[0] = q0.x; v[1] = q0.y; v[2] = q0.z; v[3] = q0.w;
+        v[4] = q1.x; v[5] = q1.y; v[6] = q1.z; v[7] = q1.w;
     } else {
 #pragma unroll
-        for (int w = 0; w < 4; ++w) {
+        for (int w = 0; w < 8; ++w) {
             uint32_t acc = 0;
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
-                uint64_t p = b0 + 4 * w + j;
-                uint32_t c = (p < len) ? (uint32_t)seq[p] : (uint32_t)'N';
+                const uint64_t p = b0 + 4 * w + j;
+                const uint32_t c = (p < len) ? (uint32_t)seq[p] : (uint32_t)'N';
                 acc |= c << (8 * j);
             }
             v[w] = acc;
         }
     }
-    uint32_t word = 0, inv = 0;
+    uint32_t word[2] = {0, 0}, inv = 0;
 #pragma unroll
-    for (int w = 0; w < 4; ++w) {
+    for (int w = 0; w < 8; ++w) {
         uint32_t i4;
-        uint32_t c8 = pack4(v[w], i4);
-        word |= c8 << (24 - 8 * w);
+        const uint32_t c8 = pack4(v[w], i4);
+        word[w >> 2] |= c8 << (24 - 8 * (w & 3));
         inv |= i4 << (4 * w);
     }
     // B of the next symbol: first flag of the next lane, or a direct byte load at the warp edge
     uint32_t nxt = __shfl_down_sync(0xFFFFFFFFu, inv & 1u, 1);
     if ((threadIdx.x & 31) == 31) {
-        uint64_t p = b0 + 16;
+        const uint64_t p = b0 + 32;
         uint32_t c = (p < len) ? (uint32_t)seq[p] : (uint32_t)'N';
         c &= 0xDFu;
         nxt = !(c == 'A' || c == 'C' || c == 'G' || c == 'T');
     }
-    uint32_t g = (k >= 2) ? (inv | (inv >> 1) | (nxt << 15)) : inv;
-    if (i < n_words_total) {
-        packed[i] = word;
-        gmask[i] = (uint16_t)g;
+    const uint32_t g = (k >= 2) ? (inv | (inv >> 1) | (nxt << 31)) : inv;
+    if (2 * i + 1 < n_words_total) {
+        *reinterpret_cast<uint2 *>(packed + 2 * i) = make_uint2(word[0], word[1]);
+        *reinterpret_cast<uint32_t *>(gmask + 2 * i) = g;
+    } else if (2 * i < n_words_total) {
+        packed[2 * i] = word[0];
+        gmask[2 * i] = (uint16_t)g;
     }
 }
 

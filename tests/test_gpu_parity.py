@@ -322,3 +322,16 @@ def test_pack_kernel_words_and_mask():
     G = inv[:-1] | inv[1:]
     want_mask = (G.reshape(nw, 16) << np.arange(16)).sum(axis=1).astype(np.uint16)
     assert np.array_equal(mask, want_mask)
+
+
+def test_every_byte_value_as_a_symbol():
+    """A9: ACGT in either case are the only valid symbols; every other byte value resets the window."""
+    rng = np.random.default_rng(11)
+    seq = seqgen.uniform(12, 400_000)
+    lower = rng.random(seq.size) < 0.3
+    seq[lower] |= 0x20                                   # lower-case a c g t are valid too
+    pos = rng.choice(seq.size, 256 * 8, replace=False)   # every byte value, 8 times, far enough apart
+    seq[pos] = np.tile(np.arange(256, dtype=np.uint8), 8)
+    q = seqgen.uniform(13, 100_000)
+    q[rng.choice(q.size, 512, replace=False)] = np.tile(np.arange(256, dtype=np.uint8), 2)
+    check_parity(DEFAULT, 1 << 24, seq, None, q, None, True)
