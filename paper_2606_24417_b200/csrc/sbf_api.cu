@@ -93,6 +93,7 @@ struct sbf {
     uint16_t *gmask;
     uint64_t cap_words;       // allocated words in packed / gmask
     uint64_t last_words;      // words written by the last pack
+    uint32_t *d_maxlen;       // longest record of the last batch (written by mark_ends_kernel)
     // L2 persistence window (a7)
     bool l2_window;
     cudaStream_t l2_stream_set;
@@ -146,7 +147,8 @@ void apply_l2_window(sbf *f, cudaStream_t st)
 }
 
 // a1: pack + validity mask (+ record ends) of one batch into the scratch
-int run_pack(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, cudaStream_t st)
+int run_pack(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, cudaStream_t st,
+             bool want_max_len = false)
 {
     int rc = ensure_scratch(f, total);
     if (rc) return rc;
@@ -158,9 +160,11 @@ int run_pack(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_
                                         aligned);
     CK(cudaGetLastError());
     g_launches++;
-    if (d_offsets && n_rec > 0 && f->k >= 2 && total > 0) {
+    if (d_offsets && n_rec > 0 && (f->k >= 2 || want_max_len) && total > 0) {
         unsigned b2 = (unsigned)((n_rec + 255) / 256);
-        mark_ends_kernel<<<b2, 256, 0, st>>>(d_offsets, n_rec, total, reinterpret_cast<uint32_t *>(f->gmask));
+        if (want_max_len) CK(cudaMemsetAsync(f->d_maxlen, 0, sizeof(uint32_t), st));
+        mark_ends_kernel<<<b2, 256, 0, st>>>(d_offsets, n_rec, total, reinterpret_cast<uint32_t *>(f->gmask), f->k,
+                                             want_max_len ? f->d_maxlen : nullptr);
         CK(cudaGetLastError());
         g_launches++;
     }
@@ -178,6 +182,7 @@ StreamParams make_params(sbf *f, uint64_t total, uint32_t *bitmap)
     p.bitmap = bitmap;
     p.n_bitmap_words = (total + 31) / 32;
     p.ones = ~0ull;
+    p.offsets = nullptr; p.n_rec = 0; p.counts = nullptr; p.max_len = nullptr; p.rec_limit = 0;
     return p;
 }
 
@@ -225,29 +230,13 @@ int run_insert(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t 
     return mark(f, 2, st);
 }
 
-int run_query(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, uint32_t *d_bitmap,
-              cudaStream_t st)
-{
-    if (total == 0) return SBF_OK;
-    apply_l2_window(f, st);
-    int rc = mark(f, 0, st);
-    if (rc) return rc;
-    rc = run_pack(f, d_bases, d_offsets, n_rec, total, st);
-    if (rc) return rc;
-    rc = mark(f, 1, st);
-    if (rc) return rc;
-    rc = run_main<false>(f, total, d_bitmap, st);
-    if (rc) return rc;
-    return mark(f, 2, st);
-}
-
 int run_count_records(const uint32_t *d_bitmap, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, uint32_t *d_counts,
-                      cudaStream_t st)
+                      cudaStream_t st, const uint32_t *max_len = nullptr, uint32_t rec_limit = 0)
 {
     if (n_rec == 0) return SBF_OK;
     if (total / n_rec < 2048) {
         unsigned blocks = (unsigned)((n_rec + 255) / 256);
-        count_records_thread_kernel<<<blocks, 256, 0, st>>>(d_bitmap, d_offsets, n_rec, d_counts);
+        count_records_thread_kernel<<<blocks, 256, 0, st>>>(d_bitmap, d_offsets, n_rec, d_counts, max_len, rec_limit);
     } else {
         unsigned blocks = (unsigned)(n_rec < 4096 ? n_rec : 4096);
         count_records_block_kernel<<<blocks, 256, 0, st>>>(d_bitmap, d_offsets, n_rec, d_counts);
@@ -255,6 +244,52 @@ int run_count_records(const uint32_t *d_bitmap, const uint64_t *d_offsets, uint6
     CK(cudaGetLastError());
     g_launches++;
     return SBF_OK;
+}
+
+// Record mode (one thread per record, stream_rec_kernel) is tried for batches of short records: the host knows only
+// the MEAN length, so the longest record is found on the device (mark_ends_kernel) and the record-mode kernel and
+// the chunk-mode kernels both look at it: exactly one of the two does the work, the other exits at once.
+constexpr uint64_t kRecMeanLimit = 400; // symbols
+constexpr uint32_t kRecMaxLimit = 1024; // symbols
+
+int run_query(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, uint32_t *d_bitmap,
+              uint32_t *d_counts, cudaStream_t st)
+{
+    if (total == 0) return SBF_OK;
+    apply_l2_window(f, st);
+    const bool try_rec = f->entry && f->entry->query_rec && d_offsets && n_rec > 0 && total / n_rec <= kRecMeanLimit;
+    int rc = mark(f, 0, st);
+    if (rc) return rc;
+    rc = run_pack(f, d_bases, d_offsets, n_rec, total, st, try_rec);
+    if (rc) return rc;
+    rc = mark(f, 1, st);
+    if (rc) return rc;
+    if (try_rec) {
+        StreamParams p = make_params(f, total, d_bitmap);
+        p.offsets = d_offsets; p.n_rec = n_rec; p.counts = d_counts; p.max_len = f->d_maxlen; p.rec_limit = kRecMaxLimit;
+        CK(cudaMemsetAsync(d_bitmap, 0, p.n_bitmap_words * sizeof(uint32_t), st)); // record mode ORs into it
+        CK(f->entry->query_rec(p, st));
+        CK(f->entry->query(p, st)); // exits at once unless a record is longer than kRecMaxLimit
+        g_launches += 2;
+        rc = mark(f, 2, st);
+        if (rc) return rc;
+        if (d_counts) {
+            rc = run_count_records(d_bitmap, d_offsets, n_rec, total, d_counts, st, f->d_maxlen, kRecMaxLimit);
+            if (rc) return rc;
+            rc = mark(f, 3, st);
+        }
+        return rc;
+    }
+    rc = run_main<false>(f, total, d_bitmap, st);
+    if (rc) return rc;
+    rc = mark(f, 2, st);
+    if (rc) return rc;
+    if (d_counts && d_offsets && n_rec) {
+        rc = run_count_records(d_bitmap, d_offsets, n_rec, total, d_counts, st);
+        if (rc) return rc;
+        rc = mark(f, 3, st);
+    }
+    return rc;
 }
 
 } // namespace
@@ -297,9 +332,11 @@ sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits)
     f->entry = find_entry(k, m, s, H);
     e = cudaMalloc(&f->filter, shards * 32);
     if (e == cudaSuccess) e = cudaMemset(f->filter, 0, shards * 32);
+    if (e == cudaSuccess) e = cudaMalloc(&f->d_maxlen, 256);
     if (e != cudaSuccess) {
         fail_cuda(e, "sbf_create: filter allocation");
         if (f->filter) cudaFree(f->filter);
+        if (f->d_maxlen) cudaFree(f->d_maxlen);
         delete f;
         return nullptr;
     }
@@ -327,6 +364,7 @@ void sbf_destroy(sbf_t *f)
     if (f->packed) cudaFree(f->packed);
     if (f->gmask) cudaFree(f->gmask);
     if (f->filter) cudaFree(f->filter);
+    if (f->d_maxlen) cudaFree(f->d_maxlen);
     cudaGetLastError();
     delete f;
 }
@@ -392,7 +430,7 @@ int sbf_query_seq(sbf_t *f, const char *d_seq, uint64_t len, uint32_t *d_bitmap,
 {
     if (!f || (!d_seq && len) || (!d_bitmap && len)) return fail(SBF_ERR_INVALID_ARG, "sbf_query_seq: NULL argument");
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = run_query(f, d_seq, nullptr, 0, len, d_bitmap, st);
+    int rc = run_query(f, d_seq, nullptr, 0, len, d_bitmap, nullptr, st);
     if (rc) return rc;
     if (d_hits) {
         CK(cudaMemsetAsync(d_hits, 0, sizeof(uint64_t), st));
@@ -416,19 +454,8 @@ int sbf_query_records(sbf_t *f, const char *d_bases, const uint64_t *d_offsets, 
         return fail(SBF_ERR_INVALID_ARG, "sbf_query_records: NULL argument");
     if (n_rec == 0 && total_bases) return fail(SBF_ERR_INVALID_ARG, "sbf_query_records: bases without records");
     cudaStream_t st = (cudaStream_t)stream;
-    int rc = run_query(f, d_bases, d_offsets, n_rec, total_bases, d_bitmap, st);
-    if (rc) return rc;
-    if (d_hit_counts && n_rec) {
-        if (total_bases == 0) {
-            CK(cudaMemsetAsync(d_hit_counts, 0, n_rec * sizeof(uint32_t), st));
-        } else {
-            rc = run_count_records(d_bitmap, d_offsets, n_rec, total_bases, d_hit_counts, st);
-            if (rc) return rc;
-            rc = mark(f, 3, st);
-            if (rc) return rc;
-        }
-    }
-    return SBF_OK;
+    if (d_hit_counts && n_rec && total_bases == 0) CK(cudaMemsetAsync(d_hit_counts, 0, n_rec * sizeof(uint32_t), st));
+    return run_query(f, d_bases, d_offsets, n_rec, total_bases, d_bitmap, d_hit_counts, st);
 }
 
 int sbf_export_bits(const sbf_t *f, void *h_dst, uint64_t nbytes)
@@ -625,7 +652,7 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
         if (insert) {
             rc = run_insert(f, R.d_bases[sl], d_off, nr, n, R.comp);
         } else {
-            rc = run_query(f, R.d_bases[sl], d_off, nr, n, R.d_bitmap + a / 32, R.comp);
+            rc = run_query(f, R.d_bases[sl], d_off, nr, n, R.d_bitmap + a / 32, nullptr, R.comp);
         }
         if (rc) return rc;
         CK(cudaEventRecord(R.computed[sl], R.comp));

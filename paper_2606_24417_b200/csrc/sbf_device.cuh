@@ -18,6 +18,9 @@
 #include <utility>
 
 // ---- tuning switches (defaults = the measured best)
+#ifndef SBF_MINB_R
+#define SBF_MINB_R 4 // record-mode query: 4 x 128 threads -> 128 registers
+#endif
 #ifndef SBF_Q_LA
 #define SBF_Q_LA 3   // query: the minimizer runs this many positions ahead of the bit tests
 #endif
@@ -60,6 +63,12 @@ struct StreamParams {
     uint32_t *bitmap;       // query: ceil(n_pos/32) words
     uint64_t n_bitmap_words;
     uint64_t ones;          // all ones (opaque to the compiler)
+    // record mode (stream_rec_kernel): one thread per record
+    const uint64_t *offsets; // n_rec + 1
+    uint64_t n_rec;
+    uint32_t *counts;        // nullable: per-record hit counts
+    const uint32_t *max_len; // device word written by mark_ends_kernel: longest record of the batch
+    uint32_t rec_limit;      // record mode runs iff *max_len <= rec_limit (the chunk kernels run otherwise)
 };
 
 struct NaiveParams {
@@ -202,15 +211,31 @@ __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ s
     }
 }
 
-// F bits: a record boundary after symbol offsets[r]-1, r = 1..n_rec  (k >= 2 only)
-__global__ void mark_ends_kernel(const uint64_t *__restrict__ offsets, uint64_t n_rec, uint64_t total, uint32_t *gmask32)
+// F bits: a record boundary after symbol offsets[r]-1, r = 1..n_rec  (k >= 2 only); also the longest
+// record of the batch -> *max_len (nullable), which selects record mode or chunk mode on the device.
+__global__ void __launch_bounds__(256) mark_ends_kernel(const uint64_t *__restrict__ offsets, uint64_t n_rec, uint64_t total,
+                                                        uint32_t *gmask32, int k, uint32_t *max_len)
 {
-    uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x + 1;
-    if (r > n_rec) return;
-    uint64_t e = offsets[r];
-    if (e == 0 || e > total) return;
-    uint64_t j = e - 1;
-    atomicOr(&gmask32[j >> 5], 1u << (j & 31));
+    __shared__ uint32_t blockMax;
+    if (threadIdx.x == 0) blockMax = 0;
+    __syncthreads();
+    const uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x + 1;
+    uint32_t len = 0;
+    if (r <= n_rec) {
+        const uint64_t e = offsets[r], a = offsets[r - 1];
+        const uint64_t l64 = e >= a ? e - a : 0;
+        len = l64 > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)l64;
+        if (k >= 2 && e != 0 && e <= total) {
+            const uint64_t j = e - 1;
+            atomicOr(&gmask32[j >> 5], 1u << (j & 31));
+        }
+    }
+    if (max_len != nullptr) {
+        len = __reduce_max_sync(0xFFFFFFFFu, len);
+        if ((threadIdx.x & 31) == 0) atomicMax(&blockMax, len);
+        __syncthreads();
+        if (threadIdx.x == 0 && blockMax) atomicMax(max_len, blockMax);
+    }
 }
 
 #endif // SBF_DEFINE_AUX_KERNELS
@@ -378,6 +403,9 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
     static_assert(Z <= 16, "stream kernel supports k-s <= 16");
     static_assert(LA >= 0 && LA <= 16 && (LA == 0 || SBF_Q_PF == 3 || 16 % LA == 0), "lookahead must divide 16");
 
+    if constexpr (!INSERT) {
+        if (prm.max_len != nullptr && __ldg(prm.max_len) <= prm.rec_limit) return; // stream_rec_kernel did this batch
+    }
     const uint64_t chunk = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint64_t p0 = chunk * kChunk;
     if (p0 >= prm.n_pos) return;
@@ -629,6 +657,188 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
 }
 
 // =============================================================================================
+// a2-a6 fused, RECORD MODE (query of short records, e.g. 150-base reads): one thread per record.
+// Same per-position arithmetic as stream_kernel<..., false> (staged shards, pair-OR masks), but the
+// thread walks exactly its record's k-mer start positions, so the K-1 tail positions of every
+// record (20 % of a 150-base read at k = 31) cost nothing, and the per-record hit count falls out of
+// the same registers.  The window is re-aligned to the record start with one funnel shift per
+// 16 symbols.  Output: the bitmap was zeroed by the caller (cudaMemsetAsync); words that lie wholly
+// inside the record are stored, the (at most two) words shared with neighbours are OR-ed in.
+// Runs only when the longest record of the batch is <= rec_limit (device flag from mark_ends_kernel);
+// otherwise every thread exits and the chunk-mode kernels, launched right after, do the work.
+// =============================================================================================
+template <int K, int M, int S, int H>
+__global__ void __launch_bounds__(kStreamTPB, SBF_MINB_R) stream_rec_kernel(const StreamParams prm)
+{
+    constexpr int WN = K - M + 1;
+    constexpr int Z = K - S;
+    constexpr int NW = H < 4 ? H : 4;
+    constexpr int RZ = ring_size(Z);
+    constexpr int L = K > 1 ? K - 1 : 1;
+    constexpr int LA = 3, NS = 4;
+    constexpr uint32_t maskL = (L >= 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
+    __shared__ uint4 stage[NS * 2 * kStreamTPB];
+
+    if (__ldg(prm.max_len) > prm.rec_limit) return;
+    const uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= prm.n_rec) return;
+    const uint64_t a = __ldg(prm.offsets + r), e = __ldg(prm.offsets + r + 1);
+    const uint32_t len = (uint32_t)(e - a);
+    const uint32_t nk = len >= (uint32_t)K ? len - K + 1 : 0; // k-mer start positions of the record
+    if (nk == 0) {
+        if (prm.counts) prm.counts[r] = 0;
+        return;
+    }
+    const uint32_t *__restrict__ pw = prm.packed + (a >> 4);
+    const uint16_t *__restrict__ gw = prm.gmask + (a >> 4);
+    const uint32_t s2 = 2u * (uint32_t)(a & 15), s1 = (uint32_t)(a & 15);
+    uint32_t rawLast;
+    uint32_t W[kWin];
+    {
+        const uint32_t r0 = __ldg(pw), r1 = __ldg(pw + 1), r2 = __ldg(pw + 2), r3 = __ldg(pw + 3);
+        rawLast = __ldg(pw + 4);
+        W[0] = __funnelshift_l(r1, r0, s2); W[1] = __funnelshift_l(r2, r1, s2);
+        W[2] = __funnelshift_l(r3, r2, s2); W[3] = __funnelshift_l(rawLast, r3, s2);
+    }
+    uint32_t glo, ghi, gLast; // G bits of positions a.. (bit 0 = position a), re-aligned like the window
+    {
+        const uint32_t g0 = (uint32_t)__ldg(gw) | ((uint32_t)__ldg(gw + 1) << 16);
+        const uint32_t g1 = (uint32_t)__ldg(gw + 2) | ((uint32_t)__ldg(gw + 3) << 16);
+        gLast = __ldg(gw + 4);
+        glo = __funnelshift_r(g0, g1, s1);
+        ghi = __funnelshift_r(g1, gLast, s1);
+    }
+
+    SlidingMin<WN> smin;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) { smin.g[i] = 0; smin.c3[i] = 0; smin.c9[i] = 0; }
+    uint64_t Mh[RZ][NW];
+#pragma unroll
+    for (int i = 0; i < RZ; ++i)
+#pragma unroll
+        for (int q = 0; q < NW; ++q) Mh[i][q] = 0;
+    static_for<0, WN - 1>([&](auto ec) {
+        constexpr int E = decltype(ec)::value;
+        (void)smin.template push<E>(g_key(lmer<E, M>(W), M));
+    });
+    static_for<0, Z>([&](auto ic) {
+        constexpr int I = decltype(ic)::value;
+        expand_masks<H, NW>(f_hash_c<S>(lmer<I, S>(W)), Mh[I % RZ]);
+    });
+    uint64_t PB[NW], PC[NW];
+#pragma unroll
+    for (int q = 0; q < NW; ++q) {
+        PB[q] = Mh[0][q] | Mh[1 % RZ][q];
+        PC[q] = Mh[1 % RZ][q] | Mh[2 % RZ][q];
+    }
+    uint32_t laPrev = 0xFFFFFFFFu;
+    bool sb[NS], laInv = true;
+#pragma unroll
+    for (int i = 0; i < NS; ++i) sb[i] = false;
+    uint64_t shard[4] = {0, 0, 0, 0};
+
+    // lookahead stage for k-mer q = (block start) + QJ: shard index, run start -> stage the sector
+    auto look = [&](auto qc) {
+        constexpr int QJ = decltype(qc)::value; // 0 .. 15+LA relative to the current window
+        const uint32_t shNew = sigma32(smin.template push<QJ + WN - 1>(g_key(lmer<QJ + WN - 1, M>(W), M)), prm.shard_shift);
+        const bool invN = (__funnelshift_r(glo, ghi, QJ) & maskL) != 0;
+        const bool start = !invN && (laInv || shNew != laPrev);
+        if (start)
+            cp_async_shard(&stage[((QJ % NS) * 2) * kStreamTPB + threadIdx.x], &stage[((QJ % NS) * 2 + 1) * kStreamTPB + threadIdx.x],
+                           prm.filter + (uint64_t)shNew * 4);
+        cp_async_commit();
+        sb[QJ % NS] = start;
+        laInv = invN;
+        laPrev = shNew;
+    };
+    static_for<0, LA>(look);
+
+    uint32_t res16 = 0;
+    auto step = [&](auto jc) {
+        constexpr int J = decltype(jc)::value;
+        look(std::integral_constant<int, J + LA>{});
+        uint64_t Mn[NW];
+        expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
+        const bool inval = (__funnelshift_r(glo, ghi, J) & maskL) != 0;
+        if (sb[J % NS]) {
+            cp_async_wait<LA>();
+            const uint4 lo = stage[((J % NS) * 2) * kStreamTPB + threadIdx.x];
+            const uint4 hi = stage[((J % NS) * 2 + 1) * kStreamTPB + threadIdx.x];
+            shard[0] = ((uint64_t)lo.y << 32) | lo.x; shard[1] = ((uint64_t)lo.w << 32) | lo.z;
+            shard[2] = ((uint64_t)hi.y << 32) | hi.x; shard[3] = ((uint64_t)hi.w << 32) | hi.z;
+        }
+        uint64_t miss = 0;
+        if constexpr (Z == 3) {
+            uint64_t mq[NW];
+#pragma unroll
+            for (int q = 0; q < NW; ++q) {
+                const uint64_t cn = Mn[q] | Mh[(J + 2) % RZ][q];
+                mq[q] = (cn | PB[q]) & ~shard[q];
+                PB[q] = PC[q];
+                PC[q] = cn;
+            }
+            if constexpr (NW == 4) miss = (mq[0] | mq[1] | mq[2]) | mq[3];
+            else
+#pragma unroll
+                for (int q = 0; q < NW; ++q) miss |= mq[q];
+        } else {
+#pragma unroll
+            for (int q = 0; q < NW; ++q) {
+                uint64_t kq_ = Mn[q];
+#pragma unroll
+                for (int i = 0; i < Z; ++i) kq_ |= Mh[(J + i) % RZ][q];
+                miss |= kq_ & ~shard[q];
+            }
+        }
+        if (!inval && miss == 0) res16 |= 1u << J;
+#pragma unroll
+        for (int q = 0; q < NW; ++q) Mh[(J + Z) % RZ][q] = Mn[q];
+    };
+
+    // result bits leave through a 64-bit buffer aligned to the bitmap's words
+    uint64_t rb = 0;
+    uint32_t fill = (uint32_t)(a & 31), cnt = 0;
+    uint64_t wi = a >> 5;
+    bool first = true;
+    auto emit = [&](uint32_t word) {
+        if (first || (wi + 1) * 32 > e) {
+            if (word) atomicOr(prm.bitmap + wi, word);
+        } else {
+            prm.bitmap[wi] = word;
+        }
+        first = false;
+        ++wi;
+    };
+
+    const uint32_t nblk = (nk + 15) >> 4;
+    for (uint32_t b = 0; b < nblk; ++b) {
+        const uint32_t rawNext = __ldg(pw + b + 5);
+        const uint32_t gNext = __ldg(gw + b + 5);
+        res16 = 0;
+        static_for<0, 8>(step);
+        if (16 * b + 8 < nk) static_for<8, 16>(step);
+        W[0] = W[1]; W[1] = W[2]; W[2] = W[3]; W[3] = __funnelshift_l(rawNext, rawLast, s2);
+        rawLast = rawNext;
+        // next 16 re-aligned G bits = bits [s1, s1+16) of gLast | gNext << 16
+        const uint32_t g16 = (__funnelshift_r(gLast | (gNext << 16), 0u, s1)) & 0xFFFFu;
+        glo = (glo >> 16) | (ghi << 16);
+        ghi = (ghi >> 16) | (g16 << 16);
+        gLast = gNext;
+        if (16 * b + 16 > nk) res16 &= (1u << (nk - 16 * b)) - 1u; // positions past the record's last k-mer
+        cnt += __popc(res16);
+        rb |= (uint64_t)res16 << fill;
+        fill += 16;
+        if (fill >= 32) {
+            emit((uint32_t)rb);
+            rb >>= 32;
+            fill -= 32;
+        }
+    }
+    if (rb) emit((uint32_t)rb);
+    if (prm.counts) prm.counts[r] = cnt;
+}
+
+// =============================================================================================
 // Runtime-parameter kernel: Alg. 1 / Alg. 2 as printed, one k-mer per thread, everything
 // recomputed per k-mer.  Serves every legal (k,m,s,H) that has no
 // specialised instance, including H > 10 (A6).  A warp covers 32 consecutive positions, so the
@@ -720,8 +930,10 @@ __device__ __forceinline__ uint32_t popc_range(const uint32_t *__restrict__ bm, 
 #ifdef SBF_DEFINE_AUX_KERNELS
 // short records: one thread per record
 __global__ void __launch_bounds__(256) count_records_thread_kernel(const uint32_t *__restrict__ bm, const uint64_t *__restrict__ offsets,
-                                                                   uint64_t n_rec, uint32_t *__restrict__ counts)
+                                                                   uint64_t n_rec, uint32_t *__restrict__ counts,
+                                                                   const uint32_t *max_len, uint32_t rec_limit)
 {
+    if (max_len != nullptr && __ldg(max_len) <= rec_limit) return; // stream_rec_kernel wrote the counts
     uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= n_rec) return;
     counts[r] = popc_range(bm, offsets[r], offsets[r + 1]);

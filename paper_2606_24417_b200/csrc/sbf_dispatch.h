@@ -14,6 +14,7 @@ struct KernelEntry {
     int k, m, s, H;
     stream_launch_fn insert;
     stream_launch_fn query;
+    stream_launch_fn query_rec; // record mode (one thread per record)
 };
 
 template <int K, int M, int S, int H, bool INSERT>
@@ -26,8 +27,18 @@ cudaError_t launch_stream(const StreamParams &prm, cudaStream_t stream)
     return cudaGetLastError();
 }
 
+template <int K, int M, int S, int H>
+cudaError_t launch_stream_rec(const StreamParams &prm, cudaStream_t stream)
+{
+    if (prm.n_rec == 0) return cudaSuccess;
+    const uint64_t blocks = (prm.n_rec + kStreamTPB - 1) / kStreamTPB;
+    stream_rec_kernel<K, M, S, H><<<(unsigned)blocks, kStreamTPB, 0, stream>>>(prm);
+    return cudaGetLastError();
+}
+
 #define SBF_ENTRY(K, M, S, H) \
-    { K, M, S, H, &sbfk::launch_stream<K, M, S, H, true>, &sbfk::launch_stream<K, M, S, H, false> }
+    { K, M, S, H, &sbfk::launch_stream<K, M, S, H, true>, &sbfk::launch_stream<K, M, S, H, false>, \
+      &sbfk::launch_stream_rec<K, M, S, H> }
 
 // one table per translation unit (compiled in parallel)
 const KernelEntry *inst_table_default(int *n);

@@ -8,7 +8,7 @@ static const KernelEntry kTable[] = {
     SBF_ENTRY(31, 16, 28, 6),
     SBF_ENTRY(31, 16, 28, 8),
 #endif
-    {0, 0, 0, 0, nullptr, nullptr}, // terminator (not counted)
+    {0, 0, 0, 0, nullptr, nullptr, nullptr}, // terminator (not counted)
 };
 const KernelEntry *inst_table_h_axis(int *n) { *n = (int)(sizeof(kTable) / sizeof(kTable[0])) - 1; return kTable; }
 } // namespace sbfk

@@ -8,7 +8,7 @@ static const KernelEntry kTable[] = {
     SBF_ENTRY(31, 18, 28, 4),
     SBF_ENTRY(31, 20, 28, 4),
 #endif
-    {0, 0, 0, 0, nullptr, nullptr}, // terminator (not counted)
+    {0, 0, 0, 0, nullptr, nullptr, nullptr}, // terminator (not counted)
 };
 const KernelEntry *inst_table_m_axis(int *n) { *n = (int)(sizeof(kTable) / sizeof(kTable[0])) - 1; return kTable; }
 } // namespace sbfk

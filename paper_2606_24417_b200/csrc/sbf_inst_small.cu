@@ -8,7 +8,7 @@ static const KernelEntry kTable[] = {
     SBF_ENTRY(21, 11, 21, 3),
     SBF_ENTRY(15, 15, 12, 5),
 #endif
-    {0, 0, 0, 0, nullptr, nullptr}, // terminator (not counted)
+    {0, 0, 0, 0, nullptr, nullptr, nullptr}, // terminator (not counted)
 };
 const KernelEntry *inst_table_small(int *n) { *n = (int)(sizeof(kTable) / sizeof(kTable[0])) - 1; return kTable; }
 } // namespace sbfk

@@ -335,3 +335,29 @@ def test_every_byte_value_as_a_symbol():
     q = seqgen.uniform(13, 100_000)
     q[rng.choice(q.size, 512, replace=False)] = np.tile(np.arange(256, dtype=np.uint8), 2)
     check_parity(DEFAULT, 1 << 24, seq, None, q, None, True)
+
+
+def test_record_mode_and_its_device_side_fallback():
+    """Short records run one-thread-per-record (stream_rec_kernel); one record above the limit makes the
+    device-side flag hand the whole batch to the chunk kernels.  Both must give the oracle's bits."""
+    seq = seqgen.markov(31, 5, 0.41, 600_000)
+    seq[1000:1100] = ord("N")
+    rng = np.random.default_rng(5)
+    # (a) ragged short records incl. empty ones, lengths 0..400, every start alignment
+    lens = rng.integers(0, 400, size=2500)
+    lens[::97] = 0
+    lens[5] = 30; lens[6] = 31; lens[7] = 32; lens[8] = 1
+    offs = np.concatenate(([0], np.cumsum(lens))).astype(np.uint64)
+    q = seqgen.reads(9, seq, 0, (int(offs[-1]) + 149) // 150, 150, 0.01)[:int(offs[-1])].copy()
+    q[rng.choice(q.size, 300, replace=False)] = ord("N")
+    check_parity(DEFAULT, 1 << 24, seq, None, q, offs, True)
+    # (b) same mean length, but one record of 5000 symbols (> 1024): chunk kernels take over
+    lens2 = lens.copy(); lens2[100] = 5000
+    offs2 = np.concatenate(([0], np.cumsum(lens2))).astype(np.uint64)
+    q2 = seqgen.reads(10, seq, 0, (int(offs2[-1]) + 149) // 150, 150, 0.01)[:int(offs2[-1])].copy()
+    check_parity(DEFAULT, 1 << 24, seq, None, q2, offs2, True)
+    # (c) fixed 150-base reads whose count is not a multiple of the CTA size, other k / H
+    for params in (dict(k=21, m=11, s=21, H=3), dict(k=31, m=16, s=28, H=8), dict(k=9, m=5, s=6, H=4)):
+        n = 1237
+        qq = seqgen.reads(11, seq, 0, n, 150, 0.02)
+        check_parity(params, 1 << 22, seq[:200_000], None, qq, seqgen.fixed_offsets(n, 150), True)
