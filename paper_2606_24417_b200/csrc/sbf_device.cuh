@@ -34,7 +34,7 @@
 #define SBF_ONEHOT 0  // one-hot masks by plain shifts (0) or through a float exponent + F2I (1; measured: no gain)
 #endif
 #ifndef SBF_MINB_I
-#define SBF_MINB_I 6 // insert: CTAs per SM the register budget is cut for (6 x 128 threads -> 80 registers)
+#define SBF_MINB_I 5 // insert: CTAs per SM the register budget is cut for (5 x 128 threads -> 96 registers)
 #endif
 #ifndef SBF_MINB_Q
 #define SBF_MINB_Q 5 // query: 5 x 128 threads -> 96 registers
@@ -50,7 +50,7 @@ constexpr uint64_t kSeedS = 0x2545F4914F6CDD1Dull;
 constexpr uint64_t kMultF = 0xD6E8FEB86659FD93ull;
 
 // ---- launch geometry ---------------------------------------------------------------------
-constexpr int kChunk = 128;     // k-mer start positions walked by one thread of stream_kernel
+constexpr int kChunk = 128;     // most k-mer start positions walked by one thread of stream_kernel (StreamParams::chunk_blocks * 16)
 constexpr int kStreamTPB = 128; // threads per CTA of stream_kernel
 constexpr int kPadWords = 16;   // zero / all-invalid words appended to the packed sequence and its mask
 
@@ -69,6 +69,7 @@ struct StreamParams {
     uint32_t *counts;        // nullable: per-record hit counts
     const uint32_t *max_len; // device word written by mark_ends_kernel: longest record of the batch
     uint32_t rec_limit;      // record mode runs iff *max_len <= rec_limit (the chunk kernels run otherwise)
+    int chunk_blocks;        // chunk mode: 16-position blocks walked by one thread (2, 4 or 8: small batches use short chunks)
 };
 
 struct NaiveParams {
@@ -407,7 +408,7 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
         if (prm.max_len != nullptr && __ldg(prm.max_len) <= prm.rec_limit) return; // stream_rec_kernel did this batch
     }
     const uint64_t chunk = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint64_t p0 = chunk * kChunk;
+    const uint64_t p0 = chunk * (uint64_t)(16 * prm.chunk_blocks);
     if (p0 >= prm.n_pos) return;
 
     const uint32_t *__restrict__ pw = prm.packed + (p0 >> 4);
@@ -483,7 +484,7 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
     bool prevInval = true; // insert: previous k-mer invalid; query: no shard loaded yet
     uint32_t res = 0;
 
-    for (int b = 0; b < kChunk / 16; ++b) {
+    for (int b = 0; b < prm.chunk_blocks; ++b) {
         const uint32_t wnext = __ldg(pw + b + 4);
         const uint32_t gnext = __ldg(gw + b + 4);
         uint32_t res16 = 0;

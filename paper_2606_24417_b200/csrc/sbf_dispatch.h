@@ -20,7 +20,8 @@ struct KernelEntry {
 template <int K, int M, int S, int H, bool INSERT>
 cudaError_t launch_stream(const StreamParams &prm, cudaStream_t stream)
 {
-    const uint64_t chunks = (prm.n_pos + kChunk - 1) / kChunk;
+    const uint64_t per = 16ull * (uint64_t)prm.chunk_blocks;
+    const uint64_t chunks = (prm.n_pos + per - 1) / per;
     if (chunks == 0) return cudaSuccess;
     const uint64_t blocks = (chunks + kStreamTPB - 1) / kStreamTPB;
     stream_kernel<K, M, S, H, INSERT><<<(unsigned)blocks, kStreamTPB, 0, stream>>>(prm);
