@@ -17,6 +17,9 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 OBJDIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsbf_b200.so")
 
+SWEEP_S = (24, 26, 28, 30, 31)   # BASELINE.json configs[4]
+SWEEP_M = (12, 14, 16, 18, 20)
+
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-std=c++17", "-O3", "-lineinfo",
@@ -47,12 +50,23 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str =
     nvcc = _nvcc()
     jobs = []
     objs = []
+    units = []  # (source, object, extra -D flags)
     for src in srcs:
-        obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+        base = os.path.basename(src)[:-3]
+        if base == "sbf_inst_sweep":
+            # one object per (s, m) pair of BASELINE config 5, five H instances each (skipped in tuning builds)
+            if "-DSBF_ONLY_DEFAULT" not in extra_flags:
+                for s_ in SWEEP_S:
+                    for m_ in SWEEP_M:
+                        units.append((src, os.path.join(objdir, "%s_s%d_m%d.o" % (base, s_, m_)),
+                                      ["-DSBF_SWEEP_S=%d" % s_, "-DSBF_SWEEP_M=%d" % m_]))
+        else:
+            units.append((src, os.path.join(objdir, base + ".o"), []))
+    for src, obj, defs in units:
         objs.append(obj)
         stale = force or not os.path.exists(obj) or os.path.getmtime(obj) < max(os.path.getmtime(src), hdr_time)
         if stale:
-            cmd = [nvcc] + NVCC_FLAGS + list(extra_flags) + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+            cmd = [nvcc] + NVCC_FLAGS + list(extra_flags) + defs + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
             jobs.append(cmd)
 
     def run(cmd):

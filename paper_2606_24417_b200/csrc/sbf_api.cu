@@ -35,17 +35,25 @@ int fail_cuda(cudaError_t e, const char *where)
         if (e__ != cudaSuccess) return fail_cuda(e__, #call);     \
     } while (0)
 
+struct TableList { // filled by the static TableRegistration objects of the sbf_inst_*.cu objects at load time
+    const KernelEntry *entries[64];
+    int counts[64];
+    int n;
+};
+TableList &tables()
+{
+    static TableList t = {};
+    return t;
+}
+
 const KernelEntry *find_entry(int k, int m, int s, int H)
 {
-    typedef const KernelEntry *(*table_fn)(int *);
-    static const table_fn tables[] = {inst_table_default, inst_table_s_axis, inst_table_m_axis, inst_table_h_axis,
-                                      inst_table_small};
-    for (table_fn t : tables) {
-        int n = 0;
-        const KernelEntry *e = t(&n);
-        for (int i = 0; i < n; ++i)
-            if (e[i].k == k && e[i].m == m && e[i].s == s && e[i].H == H) return &e[i];
-    }
+    const TableList &t = tables();
+    for (int i = 0; i < t.n; ++i)
+        for (int j = 0; j < t.counts[i]; ++j) {
+            const KernelEntry &e = t.entries[i][j];
+            if (e.k == k && e.m == m && e.s == s && e.H == H) return &e;
+        }
     return nullptr;
 }
 
@@ -81,6 +89,18 @@ struct HostRun { // persistent state of the host-facing path (two slots: copy c+
 };
 
 } // namespace
+
+namespace sbfk {
+void register_table(const KernelEntry *entries, int n)
+{
+    TableList &t = tables();
+    if (t.n < 64) {
+        t.entries[t.n] = entries;
+        t.counts[t.n] = n;
+        ++t.n;
+    }
+}
+} // namespace sbfk
 
 struct sbf {
     int k, m, s, H, P;

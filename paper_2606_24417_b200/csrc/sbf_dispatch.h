@@ -41,11 +41,10 @@ cudaError_t launch_stream_rec(const StreamParams &prm, cudaStream_t stream)
     { K, M, S, H, &sbfk::launch_stream<K, M, S, H, true>, &sbfk::launch_stream<K, M, S, H, false>, \
       &sbfk::launch_stream_rec<K, M, S, H> }
 
-// one table per translation unit (compiled in parallel)
-const KernelEntry *inst_table_default(int *n);
-const KernelEntry *inst_table_s_axis(int *n);
-const KernelEntry *inst_table_m_axis(int *n);
-const KernelEntry *inst_table_h_axis(int *n);
-const KernelEntry *inst_table_small(int *n);
+// One table per translation unit (compiled in parallel); each registers itself when the library is loaded.
+void register_table(const KernelEntry *entries, int n); // sbf_api.cu
+struct TableRegistration {
+    TableRegistration(const KernelEntry *entries, int n) { register_table(entries, n); }
+};
 
 } // namespace sbfk

@@ -129,10 +129,19 @@ def test_config5_axes_specialized(s, m, H):
     check_parity(dict(k=31, m=m, s=s, H=H), 1 << 22, w.insert_bases, None, reads, offs, expect_specialized=True)
 
 
-@pytest.mark.parametrize("s,m,H", [(24, 12, 8), (26, 20, 1), (30, 14, 6), (31, 18, 2), (24, 20, 6), (27, 8, 4),
-                                   (28, 16, 12), (28, 16, 16), (16, 4, 4), (31, 31, 4)])
-def test_config5_off_axis_runtime_kernel(s, m, H):
-    """Off-axis sweep points and H > 10 (A6) run the runtime-parameter kernel: same bits."""
+@pytest.mark.parametrize("s,m,H", [(24, 12, 8), (26, 20, 1), (30, 14, 6), (31, 18, 2), (24, 20, 6), (31, 12, 1), (26, 14, 8)])
+def test_config5_cross_product_specialized(s, m, H):
+    """Off-axis points of the 125-point cross product also have specialised instances (sbf_inst_sweep.cu)."""
+    w = seqgen.config3(scale=0.001)
+    reads = w.read_batch(0, 2000)
+    offs = seqgen.fixed_offsets(2000, 150)
+    check_parity(dict(k=31, m=m, s=s, H=H), 1 << 21, w.insert_bases, None, reads, offs, expect_specialized=True)
+    check_parity(dict(k=31, m=m, s=s, H=H), 1 << 21, w.insert_bases, None, reads[:150 * 700], None, expect_specialized=True)
+
+
+@pytest.mark.parametrize("s,m,H", [(27, 8, 4), (28, 16, 12), (28, 16, 16), (16, 4, 4), (31, 31, 4), (25, 16, 4)])
+def test_parameters_outside_the_tables_run_the_runtime_kernel(s, m, H):
+    """Any other legal (k,m,s,H), and H > 10 (A6), runs the runtime-parameter kernel: same bits."""
     w = seqgen.config3(scale=0.001)
     reads = w.read_batch(0, 2000)
     offs = seqgen.fixed_offsets(2000, 150)
