@@ -258,6 +258,7 @@ int run_count_records(const uint32_t *d_bitmap, const uint64_t *d_offsets, uint6
     if (n_rec == 0) return SBF_OK;
     if (total / n_rec < 2048) {
         unsigned blocks = (unsigned)((n_rec + 255) / 256);
+        if (max_len != nullptr && blocks > 148 * 8) blocks = 148 * 8; // fallback behind record mode: strides
         count_records_thread_kernel<<<blocks, 256, 0, st>>>(d_bitmap, d_offsets, n_rec, d_counts, max_len, rec_limit);
     } else {
         unsigned blocks = (unsigned)(n_rec < 4096 ? n_rec : 4096);

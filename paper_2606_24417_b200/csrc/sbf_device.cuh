@@ -217,9 +217,6 @@ __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ s
 __global__ void __launch_bounds__(256) mark_ends_kernel(const uint64_t *__restrict__ offsets, uint64_t n_rec, uint64_t total,
                                                         uint32_t *gmask32, int k, uint32_t *max_len)
 {
-    __shared__ uint32_t blockMax;
-    if (threadIdx.x == 0) blockMax = 0;
-    __syncthreads();
     const uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x + 1;
     uint32_t len = 0;
     if (r <= n_rec) {
@@ -232,10 +229,9 @@ __global__ void __launch_bounds__(256) mark_ends_kernel(const uint64_t *__restri
         }
     }
     if (max_len != nullptr) {
+        // one atomic per warp, and only while it can still raise the maximum (monotone, so the stale read is safe)
         len = __reduce_max_sync(0xFFFFFFFFu, len);
-        if ((threadIdx.x & 31) == 0) atomicMax(&blockMax, len);
-        __syncthreads();
-        if (threadIdx.x == 0 && blockMax) atomicMax(max_len, blockMax);
+        if ((threadIdx.x & 31) == 0 && len > *reinterpret_cast<volatile uint32_t *>(max_len)) atomicMax(max_len, len);
     }
 }
 
@@ -407,7 +403,8 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
     if constexpr (!INSERT) {
         if (prm.max_len != nullptr && __ldg(prm.max_len) <= prm.rec_limit) return; // stream_rec_kernel did this batch
     }
-    const uint64_t chunk = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // one chunk per thread; the (normally idle) fallback launch behind record mode uses a small grid and strides
+    for (uint64_t chunk = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;; chunk += (uint64_t)gridDim.x * blockDim.x) {
     const uint64_t p0 = chunk * (uint64_t)(16 * prm.chunk_blocks);
     if (p0 >= prm.n_pos) return;
 
@@ -655,6 +652,7 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
             }
         }
     }
+    } // chunk loop
 }
 
 // =============================================================================================
@@ -935,9 +933,8 @@ __global__ void __launch_bounds__(256) count_records_thread_kernel(const uint32_
                                                                    const uint32_t *max_len, uint32_t rec_limit)
 {
     if (max_len != nullptr && __ldg(max_len) <= rec_limit) return; // stream_rec_kernel wrote the counts
-    uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (r >= n_rec) return;
-    counts[r] = popc_range(bm, offsets[r], offsets[r + 1]);
+    for (uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; r < n_rec; r += (uint64_t)gridDim.x * blockDim.x)
+        counts[r] = popc_range(bm, offsets[r], offsets[r + 1]);
 }
 
 // long records: one CTA per record, grid-stride over records

@@ -23,7 +23,8 @@ cudaError_t launch_stream(const StreamParams &prm, cudaStream_t stream)
     const uint64_t per = 16ull * (uint64_t)prm.chunk_blocks;
     const uint64_t chunks = (prm.n_pos + per - 1) / per;
     if (chunks == 0) return cudaSuccess;
-    const uint64_t blocks = (chunks + kStreamTPB - 1) / kStreamTPB;
+    uint64_t blocks = (chunks + kStreamTPB - 1) / kStreamTPB;
+    if (!INSERT && prm.max_len != nullptr && blocks > 148 * 8) blocks = 148 * 8; // fallback behind record mode: strides
     stream_kernel<K, M, S, H, INSERT><<<(unsigned)blocks, kStreamTPB, 0, stream>>>(prm);
     return cudaGetLastError();
 }
