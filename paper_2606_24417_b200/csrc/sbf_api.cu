@@ -5,6 +5,7 @@
 
 #include <atomic>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -548,7 +549,7 @@ int sbf_debug_last_packed(const sbf_t *f, uint32_t *h_words, uint16_t *h_mask, u
 // =============================================================================================
 namespace {
 
-constexpr uint64_t kHostChunk = 64ull << 20; // symbols per chunk, multiple of 128
+constexpr uint64_t kHostChunk = 32ull << 20; // symbols per chunk, multiple of 128 (measured best of 8..128 Mi: DESIGN.md §6)
 
 bool is_pinned(const void *p)
 {
@@ -567,6 +568,8 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
     if (h_counts && n_rec) memset(h_counts, 0, n_rec * sizeof(uint32_t));
     if (h_hits) *h_hits = 0;
     if (total == 0) return SBF_OK;
+    // the internal streams are non-blocking: order this call after everything the caller enqueued before it
+    CK(cudaDeviceSynchronize());
     const uint64_t ov = (uint64_t)f->k - 1;
     const uint64_t span = (total < kHostChunk ? total : kHostChunk) + ov; // largest chunk incl. overlap
     const uint64_t n_chunks = (total + kHostChunk - 1) / kHostChunk;
