@@ -202,7 +202,6 @@ StreamParams make_params(sbf *f, uint64_t total, uint32_t *bitmap)
     p.shard_shift = 32 - f->P;
     p.bitmap = bitmap;
     p.n_bitmap_words = (total + 31) / 32;
-    p.ones = ~0ull;
     // short chunks for small batches, so that the grid still fills 148 SMs x 6 CTAs a few times over
     p.chunk_blocks = total >= (64ull << 20) ? 8 : total >= (16ull << 20) ? 4 : 2;
     p.offsets = nullptr; p.n_rec = 0; p.counts = nullptr; p.max_len = nullptr; p.rec_limit = 0;

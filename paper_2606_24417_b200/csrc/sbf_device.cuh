@@ -25,13 +25,7 @@
 #define SBF_Q_LA 3   // query: the minimizer runs this many positions ahead of the bit tests
 #endif
 #ifndef SBF_Q_PF
-#define SBF_Q_PF 3   // query: 0 no prefetch, 1 prefetch.global.L2, 2 prefetch.global.L1, 3 cp.async staging in shared memory
-#endif
-#ifndef SBF_I_VAR
-#define SBF_I_VAR 0  // insert: accumulator scheme (see stream_kernel)
-#endif
-#ifndef SBF_ONEHOT
-#define SBF_ONEHOT 0  // one-hot masks by plain shifts (0) or through a float exponent + F2I (1; measured: no gain)
+#define SBF_Q_PF 3   // query (chunk mode): 0 load at first use, 1 prefetch.global.L2 ahead, 3 cp.async staging in shared memory
 #endif
 #ifndef SBF_MINB_I
 #define SBF_MINB_I 5 // insert: CTAs per SM the register budget is cut for (5 x 128 threads -> 96 registers)
@@ -62,7 +56,6 @@ struct StreamParams {
     int shard_shift;        // 32 - P
     uint32_t *bitmap;       // query: ceil(n_pos/32) words
     uint64_t n_bitmap_words;
-    uint64_t ones;          // all ones (opaque to the compiler)
     // record mode (stream_rec_kernel): one thread per record
     const uint64_t *offsets; // n_rec + 1
     uint64_t n_rec;
@@ -305,29 +298,11 @@ struct SlidingMin {
     }
 };
 
-// One-hot sector masks of one s-mer hash: hash index i -> word i mod 4, bit B(h,i) (A5).
-// SBF_ONEHOT == 1 builds 1 << b off the saturated ALU pipe: the 6 bits of b are moved into the exponent
-// field of a float (2^(b+1), one LOP3), halved on the FMA pipe and converted with one F2I.U64 (XU pipe);
-// every step is exact.  SBF_ONEHOT == 0 is the plain shift form (two SHF per bit on the ALU pipe).
+// One-hot sector masks of one s-mer hash: hash index i -> word i mod 4, bit B(h,i) (A5)
 template <int OFF>
 __device__ __forceinline__ uint64_t onehot_at(uint64_t h)
 {
-#if SBF_ONEHOT == 1
-    constexpr int o = OFF % 32;
-    if constexpr (o + 6 <= 32) {
-        const uint32_t half = OFF < 32 ? (uint32_t)h : (uint32_t)(h >> 32);
-        uint32_t t;
-        if constexpr (o <= 23) t = half << (23 - o);
-        else t = half >> (o - 23);
-        const float f = __uint_as_float((t & 0x1F800000u) | 0x40000000u) * 0.5f; // 2^b
-        return __float2ull_rz(f);
-    } else {
-        const uint32_t b = (uint32_t)(h >> OFF) & 63u;
-        return __float2ull_rz(__uint_as_float((b << 23) | 0x40000000u) * 0.5f);
-    }
-#else
     return 1ull << ((h >> OFF) & 63);
-#endif
 }
 
 template <int H, int NW>
@@ -366,11 +341,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 
 __device__ __forceinline__ void prefetch_shard(const uint64_t *p)
 {
-#if SBF_Q_PF == 2
-    asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
-#else
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-#endif
 }
 
 // =============================================================================================
@@ -515,57 +486,11 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
             const bool inval = (__funnelshift_r(glo, ghi, J) & maskL) != 0;
             if constexpr (INSERT) {
                 const bool brk = (sh != prevShard) || (inval != prevInval);
-#if SBF_I_VAR == 3
-                // acc = s-mers [run start, p-1]; the run's last k-mer p-1 also owns the Z s-mers p .. p+Z-1
-                if (brk && !prevInval) { // a5: flush the finished run
-                    uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
-#pragma unroll
-                    for (int q = 0; q < NW; ++q) {
-                        uint64_t o = acc[q];
-#pragma unroll
-                        for (int i = 0; i < Z; ++i) o |= Mh[(J + i) % RZ][q];
-                        red_or_64(dst + q, o);
-                    }
-                }
-                {
-                    const uint64_t keep = brk ? 0ull : ~0ull;
-#pragma unroll
-                    for (int q = 0; q < NW; ++q) acc[q] = (acc[q] & keep) | (Z > 0 ? Mh[J % RZ][q] : Mn[q]);
-                }
-#elif SBF_I_VAR == 2
-                // branch-free: K = mask of k-mer p; acc restarts from K at a break
-                uint64_t Kq[NW];
-#pragma unroll
-                for (int q = 0; q < NW; ++q) {
-                    uint64_t r = Mn[q];
-#pragma unroll
-                    for (int i = 0; i < Z; ++i) r |= Mh[(J + i) % RZ][q];
-                    Kq[q] = r;
-                }
-                if (brk && !prevInval) {
-                    uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
-#pragma unroll
-                    for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
-                }
-                {
-                    const uint64_t keep = brk ? 0ull : ~0ull;
-#pragma unroll
-                    for (int q = 0; q < NW; ++q) acc[q] = (acc[q] & keep) | Kq[q];
-                }
-#else
                 if (brk) {
                     if (!prevInval) { // a5: flush the finished run
                         uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
-#if SBF_I_VAR == 1
-                        uint64_t o[NW];
-#pragma unroll
-                        for (int q = 0; q < NW; ++q) o[q] = acc[q] & prm.ones;
-#pragma unroll
-                        for (int q = 0; q < NW; ++q) red_or_64(dst + q, o[q]);
-#else
 #pragma unroll
                         for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
-#endif
                     }
 #pragma unroll
                     for (int q = 0; q < NW; ++q) { // restart with the k-s s-mers shared with the previous k-mers
@@ -577,7 +502,6 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
                 }
 #pragma unroll
                 for (int q = 0; q < NW; ++q) acc[q] |= Mn[q];
-#endif
                 prevShard = sh;
                 prevInval = inval;
             } else {
@@ -642,12 +566,7 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
             uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
 #pragma unroll
             for (int q = 0; q < NW; ++q) {
-                uint64_t o = acc[q];
-#if SBF_I_VAR == 3
-                // after the loop the ring holds s-mers pEnd .. pEnd+Z-1 at slots (i % RZ), pEnd = 0 mod 16
-#pragma unroll
-                for (int i = 0; i < Z; ++i) o |= Mh[i % RZ][q];
-#endif
+                const uint64_t o = acc[q];
                 red_or_64(dst + q, o);
             }
         }
