@@ -71,6 +71,8 @@ def make_workload(name: str, rank: int, scale: float):
         w = seqgen.config1()
         w.n_reads = 6000
         w.read_seed = 3
+    elif name == "config4":
+        w = seqgen.config4(scale=scale)
     else:
         raise SystemExit("unknown workload %r" % name)
     if rank:  # weak scaling: every rank owns an independent sequence of the same recipe
@@ -81,6 +83,9 @@ def make_workload(name: str, rank: int, scale: float):
         elif name == "config2":
             seq = seqgen.markov(21 + 1000 * rank, 3, 0.50, n)
             seqgen.plant_copies(22 + 1000 * rank, seq, max(1, int(200 * scale)), 1000, 5000, 0.005)
+        elif name == "config4":
+            seq = seqgen.markov(41 + 1000 * rank, 5, 0.41, n)
+            seqgen.plant_families(42 + 1000 * rank, seq, [300] * 6 + [6000] * 2, 0.05, 0.10, 0.20)
         else:
             seq = seqgen.uniform(1 + 1000 * rank, n)
         w.insert_bases = seq
@@ -268,7 +273,10 @@ def run_cuda(args):
     p = w.params
     k = p["k"]
     seq_h = torch.from_numpy(w.insert_bases).pin_memory()
-    n_ins_kmers = count_valid_kmers_seq(w.insert_bases, k)
+    ins_offs_np = np.ascontiguousarray(w.insert_offsets, dtype=np.uint64)
+    n_ins_rec = ins_offs_np.size - 1
+    n_ins_kmers = sum(count_valid_kmers_seq(w.insert_bases[int(ins_offs_np[r]):int(ins_offs_np[r + 1])], k)
+                      for r in range(n_ins_rec))
     rb = min(args.read_batch, max(w.n_reads, 1))
     n_batches = max(1, min(args.batches, max(w.n_reads, 1) // rb))
     offs_np = seqgen.fixed_offsets(rb, w.read_len)
@@ -281,6 +289,13 @@ def run_cuda(args):
     offs_h = torch.from_numpy(offs_np.view(np.int64)).pin_memory()
 
     d_seq = seq_h.cuda(non_blocking=True)
+    d_ins_offs = torch.from_numpy(ins_offs_np.view(np.int64)).cuda()
+
+    def do_insert(st):  # one sequence, or a dense record batch (config 4)
+        if n_ins_rec == 1:
+            sbf.sbf_insert_seq(h, d_seq, d_seq.numel(), st)
+        else:
+            sbf.sbf_insert_records(h, d_seq, d_ins_offs, n_ins_rec, d_seq.numel(), st)
     d_reads = [t.cuda(non_blocking=True) for t in reads_h]
     d_offs = offs_h.cuda(non_blocking=True)
     n_read_bases = rb * w.read_len
@@ -300,7 +315,7 @@ def run_cuda(args):
         b = i % n_batches
         if ev: ev[0].record(stream)
         sbf.sbf_clear(h, stream)
-        sbf.sbf_insert_seq(h, d_seq, d_seq.numel(), stream)
+        do_insert(stream)
         if world > 1:
             replicas.or_allreduce_filter(h, stream=stream)
         if ev: ev[1].record(stream)
@@ -346,7 +361,7 @@ def run_cuda(args):
     for i in range(min(args.steps, 5)):
         b = (args.warmup + i) % n_batches
         sbf.sbf_clear(h, stream)
-        sbf.sbf_insert_seq(h, d_seq, d_seq.numel(), stream)
+        do_insert(stream)
         pk, mn, _ = sbf.sbf_get_timing(h)
         ins_kernel_ms.append(mn); pack_ms.append(pk)
         sbf.sbf_query_records(h, d_reads[b], d_offs, rb, n_read_bases, d_bitmap, d_counts, stream)
@@ -368,7 +383,10 @@ def run_cuda(args):
     def e2e_step(i):
         b = i % n_batches
         sbf.sbf_clear(h, None)
-        sbf.sbf_insert_seq_host(h, seq_h, seq_h.numel())
+        if n_ins_rec == 1:
+            sbf.sbf_insert_seq_host(h, seq_h, seq_h.numel())
+        else:
+            sbf.sbf_insert_records_host(h, seq_h, ins_offs_np, n_ins_rec)
         if world > 1:
             replicas.or_allreduce_filter(h, stream=stream)
             torch.cuda.synchronize()
@@ -443,7 +461,7 @@ def run_cuda(args):
             "dtype": "u64", "data": "synthetic",
             "config": {"workload": args.workload, "k": k, "m": p["m"], "s": p["s"], "H": p["H"],
                        "filter_bits": num_bits, "insert_bases_per_rank": int(d_seq.numel()),
-                       "insert_kmers_per_rank": int(n_ins_kmers), "reads_per_batch": rb, "read_len": w.read_len,
+                       "insert_kmers_per_rank": int(n_ins_kmers), "insert_records": int(n_ins_rec), "reads_per_batch": rb, "read_len": w.read_len,
                        "read_batches": n_batches, "l2": "inputs larger than L2 (sequence %d MB, read batch %d MB, "
                        "filter %d MiB); no flush" % (d_seq.numel() // 10**6, n_read_bases // 10**6, num_bits >> 23),
                        "parallelism": "replicas x%d + OR all-reduce" % world if world > 1 else "single GPU"},
@@ -501,7 +519,7 @@ def main():
     ap.add_argument("--steps", type=int, default=40)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3"])
+    ap.add_argument("--workload", default="config3", choices=["config1", "config2", "config3", "config4"])
     ap.add_argument("--scale", type=float, default=1.0, help="shrink the workload (tests only)")
     ap.add_argument("--read-batch", type=int, default=4_000_000, help="reads per query batch (one per step)")
     ap.add_argument("--batches", type=int, default=4, help="distinct read batches rotated over the steps")

@@ -127,3 +127,34 @@ def test_timing_abi_reports_kernel_times():
         n0 = sbf.sbf_kernel_launches()
         f.insert_seq(d)
         assert sbf.sbf_kernel_launches() - n0 == 2   # pack + fused insert kernel
+
+
+def test_config4_full_size_insert_and_query_batch():
+    """BASELINE config 4 at full size: 3.1 Gbp in 24 records into a 2^35-bit filter (every one of the 4 GiB filter
+    bytes compared), then one 4e6-read batch (bitmap and counts compared)."""
+    w = seqgen.config4()
+    nb = w.params["num_bits"]
+    o = oracle.OracleSBF(num_bits=nb, **DEFAULT)
+    n_ins = o.insert_records(w.insert_bases, w.insert_offsets, threads=True)
+    assert n_ins > 3_000_000_000
+    n_reads = 4_000_000
+    reads = w.read_batch(0, n_reads)
+    offs = seqgen.fixed_offsets(n_reads, w.read_len)
+    with sbf.SuperBloomFilter(num_bits=nb, **DEFAULT) as f:
+        assert f.num_shards == o.num_shards == 1 << 27
+        f.insert_records(_dev(w.insert_bases), _dev(w.insert_offsets.view(np.int64)))
+        torch.cuda.synchronize()
+        got = f.export_bits()
+        want = o.words().reshape(-1).view(np.uint8)
+        step = 1 << 28
+        for a in range(0, got.size, step):                  # compare in slices: no third 4 GiB copy
+            _first_diff(got[a:a + step], want[a:a + step], "filter bytes [%d, +%d)" % (a, step))
+        del got
+        bm = torch.full(((reads.size + 31) // 32,), -1, dtype=torch.int32, device="cuda")
+        hc = torch.full((n_reads,), -1, dtype=torch.int32, device="cuda")
+        f.query_records(_dev(reads), _dev(offs.view(np.int64)), bm, hc)
+        torch.cuda.synchronize()
+        wbm, wc, _ = o.query_records(reads, offs, threads=True)
+        _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "bitmap words")
+        _first_diff(hc.cpu().numpy().view(np.uint32), wc, "hit counts")
+    o.close()
