@@ -379,6 +379,7 @@ def run_cuda(args):
     sbf.sbf_set_timing(h, False)
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     hb_np, hc_np = h_bitmap.numpy().view(np.uint32), h_counts.numpy().view(np.uint32)
+    offs_pinned_np = offs_h.numpy().view(np.uint64)  # offsets, like every other host buffer of this leg, are pinned
 
     def e2e_step(i):
         b = i % n_batches
@@ -390,7 +391,7 @@ def run_cuda(args):
         if world > 1:
             replicas.or_allreduce_filter(h, stream=stream)
             torch.cuda.synchronize()
-        sbf.sbf_query_records_host(h, reads_h[b], offs_np, rb, hb_np, hc_np)
+        sbf.sbf_query_records_host(h, reads_h[b], offs_pinned_np, rb, hb_np, hc_np)
         return b
 
     e2e_step(0)

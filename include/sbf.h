@@ -120,7 +120,9 @@ int sbf_query_records(sbf_t *f, const char *d_bases, const uint64_t *d_offsets, 
  * chunks, overlapping the copies with the kernels on two internal streams,
  * and returns after everything has completed.  A host-facing call first waits for all work enqueued on the device
  * before it (cudaDeviceSynchronize), so it may follow device-facing calls on any stream.
- * h_bitmap / h_hit_counts as above, on the host.
+ * h_bitmap / h_hit_counts as above, on the host.  For full PCIe speed every host buffer, h_offsets included, should be
+ * pinned (cudaHostAlloc / cudaHostRegister): pageable symbols are staged through pinned buffers, pageable offsets and
+ * results are copied at pageable speed.
  */
 int sbf_insert_seq_host(sbf_t *f, const char *h_seq, uint64_t len);
 int sbf_insert_records_host(sbf_t *f, const char *h_bases, const uint64_t *h_offsets, uint64_t n_rec);

@@ -3,6 +3,7 @@
 // runs in the kernels of sbf_device.cuh; this file only sizes buffers and enqueues launches.
 #include "../../include/sbf.h"
 
+#include <algorithm>
 #include <atomic>
 #include <cstdio>
 #include <cstdlib>
@@ -60,10 +61,9 @@ const KernelEntry *find_entry(int k, int m, int s, int H)
 
 struct HostRun { // persistent state of the host-facing path (two slots: copy c+1 while computing c)
     cudaStream_t copy = nullptr, comp = nullptr;
-    cudaEvent_t copied[2] = {nullptr, nullptr}, computed[2] = {nullptr, nullptr};
+    cudaEvent_t copied[2] = {nullptr, nullptr}, computed[2] = {nullptr, nullptr}, offs_ready = nullptr;
     char *pin[2] = {nullptr, nullptr};     // pinned staging for symbols (pageable caller memory only)
     char *d_bases[2] = {nullptr, nullptr};
-    uint64_t *h_off[2] = {nullptr, nullptr};
     uint64_t *d_off[2] = {nullptr, nullptr};
     uint64_t cap_pin = 0, cap_bases = 0, cap_off = 0;
     uint32_t *d_bitmap = nullptr;  uint64_t cap_bitmap = 0;
@@ -75,10 +75,10 @@ struct HostRun { // persistent state of the host-facing path (two slots: copy c+
             if (copied[i]) cudaEventDestroy(copied[i]);
             if (computed[i]) cudaEventDestroy(computed[i]);
             if (pin[i]) cudaFreeHost(pin[i]);
-            if (h_off[i]) cudaFreeHost(h_off[i]);
             if (d_bases[i]) cudaFree(d_bases[i]);
             if (d_off[i]) cudaFree(d_off[i]);
         }
+        if (offs_ready) cudaEventDestroy(offs_ready);
         if (d_bitmap) cudaFree(d_bitmap);
         if (d_off_full) cudaFree(d_off_full);
         if (d_counts) cudaFree(d_counts);
@@ -564,9 +564,11 @@ bool is_pinned(const void *p)
 int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets, uint64_t n_rec, uint64_t total,
              uint32_t *h_bitmap, uint32_t *h_counts, uint64_t *h_hits)
 {
-    if (h_counts && n_rec) memset(h_counts, 0, n_rec * sizeof(uint32_t));
     if (h_hits) *h_hits = 0;
-    if (total == 0) return SBF_OK;
+    if (total == 0) {
+        if (h_counts && n_rec) memset(h_counts, 0, n_rec * sizeof(uint32_t));
+        return SBF_OK;
+    }
     // the internal streams are non-blocking: order this call after everything the caller enqueued before it
     CK(cudaDeviceSynchronize());
     const uint64_t ov = (uint64_t)f->k - 1;
@@ -586,6 +588,7 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
             CK(cudaEventCreateWithFlags(&f->host->copied[i], cudaEventDisableTiming));
             CK(cudaEventCreateWithFlags(&f->host->computed[i], cudaEventDisableTiming));
         }
+        CK(cudaEventCreateWithFlags(&f->host->offs_ready, cudaEventDisableTiming));
     }
     HostRun &R = *f->host;
     const int slots = n_chunks > 1 ? 2 : 1;
@@ -609,16 +612,25 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
     }
     if (h_offsets && R.cap_off < max_off) {
         for (int i = 0; i < 2; ++i) {
-            if (R.h_off[i]) cudaFreeHost(R.h_off[i]);
             if (R.d_off[i]) cudaFree(R.d_off[i]);
-            R.h_off[i] = nullptr; R.d_off[i] = nullptr;
+            R.d_off[i] = nullptr;
         }
         R.cap_off = 0;
-        for (int i = 0; i < 2; ++i) {
-            CK(cudaMallocHost(&R.h_off[i], max_off * sizeof(uint64_t)));
-            CK(cudaMalloc(&R.d_off[i], max_off * sizeof(uint64_t)));
-        }
+        for (int i = 0; i < 2; ++i) CK(cudaMalloc(&R.d_off[i], max_off * sizeof(uint64_t)));
         R.cap_off = max_off;
+    }
+    if (h_offsets) { // the batch's offsets go to the device ONCE; every chunk's own offsets are derived from them there
+        if (R.cap_rec < n_rec + 1) {
+            if (R.d_off_full) cudaFree(R.d_off_full);
+            if (R.d_counts) cudaFree(R.d_counts);
+            R.d_off_full = nullptr; R.d_counts = nullptr; R.cap_rec = 0;
+            CK(cudaMalloc(&R.d_off_full, (n_rec + 1) * sizeof(uint64_t)));
+            CK(cudaMalloc(&R.d_counts, (n_rec + 1) * sizeof(uint32_t)));
+            R.cap_rec = n_rec + 1;
+        }
+        CK(cudaMemcpyAsync(R.d_off_full, h_offsets, (n_rec + 1) * sizeof(uint64_t), cudaMemcpyHostToDevice, R.copy));
+        CK(cudaEventRecord(R.offs_ready, R.copy));
+        CK(cudaStreamWaitEvent(R.comp, R.offs_ready, 0));
     }
     (void)slots;
     const uint64_t n_bm = (total + 31) / 32;
@@ -628,17 +640,6 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
             R.d_bitmap = nullptr; R.cap_bitmap = 0;
             CK(cudaMalloc(&R.d_bitmap, (n_bm + 4) * sizeof(uint32_t)));
             R.cap_bitmap = n_bm + 4;
-        }
-        if (h_counts && n_rec) {
-            if (R.cap_rec < n_rec) {
-                if (R.d_off_full) cudaFree(R.d_off_full);
-                if (R.d_counts) cudaFree(R.d_counts);
-                R.d_off_full = nullptr; R.d_counts = nullptr; R.cap_rec = 0;
-                CK(cudaMalloc(&R.d_off_full, (n_rec + 1) * sizeof(uint64_t)));
-                CK(cudaMalloc(&R.d_counts, n_rec * sizeof(uint32_t)));
-                R.cap_rec = n_rec;
-            }
-            CK(cudaMemcpyAsync(R.d_off_full, h_offsets, (n_rec + 1) * sizeof(uint64_t), cudaMemcpyHostToDevice, R.copy));
         }
         if (h_hits && !R.d_hits) CK(cudaMalloc(&R.d_hits, sizeof(unsigned long long)));
     }
@@ -657,12 +658,16 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
         }
         uint64_t n_off = 0;
         if (h_offsets) {
-            while (off_lo <= n_rec && h_offsets[off_lo] <= a) ++off_lo;
-            uint64_t *ho = R.h_off[sl];
-            ho[n_off++] = 0;
-            for (uint64_t i = off_lo; i <= n_rec && h_offsets[i] < e; ++i) ho[n_off++] = h_offsets[i] - a;
-            ho[n_off++] = n;
-            CK(cudaMemcpyAsync(R.d_off[sl], ho, n_off * sizeof(uint64_t), cudaMemcpyHostToDevice, R.copy));
+            // record boundaries strictly inside (a, e): indices [lo, hi) of the batch's offsets
+            const uint64_t *lo = std::upper_bound(h_offsets + off_lo, h_offsets + n_rec + 1, a);
+            const uint64_t *hi = std::lower_bound(lo, h_offsets + n_rec + 1, e);
+            off_lo = (uint64_t)(lo - h_offsets);
+            const uint64_t n_inner = (uint64_t)(hi - lo);
+            n_off = n_inner + 2;
+            rebase_offsets_kernel<<<(unsigned)((n_inner + 256) / 256), 256, 0, R.comp>>>(R.d_off_full + off_lo, n_inner, a, n,
+                                                                                       R.d_off[sl]);
+            CK(cudaGetLastError());
+            g_launches++;
         }
         const char *src = h_bases + a;
         if (!direct) {

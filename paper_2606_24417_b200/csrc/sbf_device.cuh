@@ -894,6 +894,19 @@ __global__ void __launch_bounds__(256) count_total_kernel(const uint32_t *__rest
     if ((threadIdx.x & 31) == 0 && c) atomicAdd(hits, c);
 }
 
+// host-facing path: offsets of one chunk [a, a+n) of a batch from the batch's offsets (already on the device):
+// out = {0, full[0]-a, ..., full[n_inner-1]-a, n}, full pointing at the first boundary inside the chunk
+__global__ void __launch_bounds__(256) rebase_offsets_kernel(const uint64_t *__restrict__ full, uint64_t n_inner, uint64_t a, uint64_t n,
+                                                             uint64_t *__restrict__ out)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) {
+        out[0] = 0;
+        out[n_inner + 1] = n;
+    }
+    if (i < n_inner) out[1 + i] = full[i] - a;
+}
+
 // filter |= src  (replica merge)
 __global__ void __launch_bounds__(256) or_words_kernel(uint64_t *__restrict__ dst, const uint64_t *__restrict__ src, uint64_t n_words)
 {
