@@ -3,8 +3,8 @@
 The path shards by input: every rank owns a private filter replica and a contiguous slice of the
 insert batch (k-mer start positions, or whole records); after the local inserts ONE exchange step
 makes the replicas identical — a bitwise-OR all-reduce of the filter bytes.  NCCL has no OR
-reduction, so it is an all-gather of (a window of) the replicas followed by the library's
-``sbf_or_bits_device`` kernel.  Queries then shard by reads with no collective at all.
+reduction, so it is a reduce-scatter built from point-to-point exchanges plus the library's
+``sbf_or_range_device`` kernel, followed by an in-place all-gather.  Queries then shard by reads with no collective at all.
 
 Only argument marshalling and ``torch.distributed`` calls live here; nothing of the filter's
 arithmetic.  The partition helpers are pure functions so that world_size-2 gloo tests can check
@@ -56,15 +56,24 @@ def rebase_offsets(offsets: np.ndarray, r0: int, r1: int) -> np.ndarray:
     return (off[r0:r1 + 1] - off[r0]).astype(np.uint64)
 
 
-def or_allreduce(local, or_into: Callable[[object], None], group=None, window_bytes: int = 1 << 28) -> int:
-    """Make every rank's replica the OR of all replicas.
+def _slices(n: int, world: int):
+    """Cut [0, n) (n a multiple of 32) in `world` contiguous slices on 32-byte (shard) boundaries."""
+    shards = n // 32
+    cuts = [32 * ((shards * r) // world) for r in range(world + 1)]
+    return [(cuts[r], cuts[r + 1]) for r in range(world)]
 
-    local    : 1-D uint8 torch tensor viewing this rank's replica (device tensor under NCCL,
-               CPU tensor under gloo); read during the gathers, updated by ``or_into``.
-    or_into  : callable(offset_bytes, peer_chunk_tensor) that ORs a peer's chunk into the local
-               replica at that byte offset (sbf_or_bits_device on a sub-range for the GPU path).
-    The replicas are exchanged window by window so the gather buffer stays at
-    world * window_bytes (a 4 GiB filter on 8 ranks would otherwise need 32 GiB of scratch).
+
+def or_allreduce(local, or_into: Callable[[int, object], None], group=None, window_bytes: int = 1 << 28) -> int:
+    """Make every rank's replica the OR of all replicas — a reduce-scatter followed by an all-gather, so that
+    each rank sends and receives 2 (N-1)/N of the filter instead of the N-1 filters of a plain all-gather.
+
+    local    : 1-D uint8 torch tensor viewing this rank's replica (device tensor under NCCL, CPU tensor under
+               gloo), a multiple of 32 bytes long; updated in place.
+    or_into  : callable(offset_bytes, peer_chunk_tensor) that ORs a peer's chunk into the local replica at that
+               byte offset (sbf_or_range_device for the GPU path).
+    Per window of the filter (scratch stays at window_bytes): (1) every rank sends slice j of its window to rank j
+    (batched point-to-point) and ORs the N-1 slices it receives into its own slice; (2) the now final slices are
+    all-gathered straight into the local replica (no kernel: the gather's outputs ARE views of the filter).
     Returns the number of OR calls issued.
     """
     import torch
@@ -75,18 +84,49 @@ def or_allreduce(local, or_into: Callable[[object], None], group=None, window_by
     if world == 1:
         return 0
     n = local.numel()
-    window = min(n, max(32, window_bytes - window_bytes % 32))
-    gathered = torch.empty(world * window, dtype=torch.uint8, device=local.device)
+    assert n % 32 == 0, "the filter is a whole number of 32-byte shards"
+    window = min(n, max(32 * world, window_bytes - window_bytes % 32))
+    scratch = torch.empty(window, dtype=torch.uint8, device=local.device)
     calls = 0
     for a in range(0, n, window):
         w = min(window, n - a)
-        outs: List = [gathered[r * window:r * window + w] for r in range(world)]
-        dist.all_gather(outs, local[a:a + w].contiguous(), group=group)
-        for r in range(world):
-            if r != rank:
-                or_into(a, outs[r])
-                calls += 1
+        sl = _slices(w, world)
+        my0, my1 = sl[rank]
+        # (1) reduce-scatter: my slice of every peer's window arrives in scratch, one peer after the other
+        ops, views, pos = [], [], 0
+        for peer in range(world):
+            if peer == rank:
+                continue
+            p0, p1 = sl[peer]
+            if p1 > p0:
+                ops.append(dist.P2POp(dist.isend, local[a + p0:a + p1], _global_rank(group, peer), group))
+            if my1 > my0:
+                v = scratch[pos:pos + (my1 - my0)]
+                pos += my1 - my0
+                views.append(v)
+                ops.append(dist.P2POp(dist.irecv, v, _global_rank(group, peer), group))
+        if ops:
+            for req in dist.batch_isend_irecv(ops):
+                req.wait()
+        for v in views:
+            or_into(a + my0, v)
+            calls += 1
+        # (2) all-gather of the reduced slices, in place (slices may differ in length by one shard: gather by broadcast
+        #     when they do, by one all_gather when they are equal)
+        lens = {p1 - p0 for p0, p1 in sl}
+        if len(lens) == 1 and my1 > my0:
+            dist.all_gather([local[a + p0:a + p1] for p0, p1 in sl], local[a + my0:a + my1].clone(), group=group)
+        else:
+            for src in range(world):
+                p0, p1 = sl[src]
+                if p1 > p0:
+                    dist.broadcast(local[a + p0:a + p1], _global_rank(group, src), group=group)
     return calls
+
+
+def _global_rank(group, group_rank: int) -> int:
+    import torch.distributed as dist
+    return group_rank if group is None else dist.get_global_rank(group, group_rank)
 
 
 class DevicePtrView:

@@ -32,7 +32,7 @@ def _workload():
     return seq, offs
 
 
-def _rank_main(rank, world, port, mode, out_dir):
+def _rank_main(rank, world, port, mode, out_dir, window=40_000):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
@@ -55,17 +55,17 @@ def _rank_main(rank, world, port, mode, out_dir):
             dst = words.view(np.uint8)[offset:offset + c.size]
             np.bitwise_or(dst, c, out=dst)
 
-        calls = replicas.or_allreduce(local, or_into, window_bytes=40_000)  # several windows, last one ragged
-        assert calls == (world - 1) * -(-local.numel() // (40_000 - 40_000 % 32))
+        calls = replicas.or_allreduce(local, or_into, window_bytes=window)  # several windows, last one ragged
+        assert calls == (world - 1) * -(-local.numel() // (window - window % 32))  # one OR per peer per window
         np.save(os.path.join(out_dir, "rank%d.npy" % rank), o.export_bits())
     finally:
         dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("mode", ["positions", "records"])
-def test_partition_plus_or_allreduce_equals_single_rank(tmp_path, mode):
-    world = 2
-    mp.spawn(_rank_main, args=(world, _free_port(), mode, str(tmp_path)), nprocs=world, join=True)
+@pytest.mark.parametrize("mode,world,window", [("positions", 2, 40_000), ("records", 2, 65_536), ("positions", 3, 40_000),
+                                               ("records", 4, 16_384)])
+def test_partition_plus_or_allreduce_equals_single_rank(tmp_path, mode, world, window):
+    mp.spawn(_rank_main, args=(world, _free_port(), mode, str(tmp_path), window), nprocs=world, join=True)
     seq, offs = _workload()
     ref = oracle.OracleSBF(num_bits=NUM_BITS, **P)
     if mode == "positions":
