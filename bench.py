@@ -487,13 +487,18 @@ def run_cuda(args):
 
 def load_traffic(kernel: str):
     """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
-    (profiles/traffic.json, written by hand from the .ncu-rep; null until a capture exists)."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    (profiles/traffic.csv, written from the .ncu-rep's dram__bytes_read.sum + dram__bytes_write.sum; see
+    profiles/ncu_full_r01.md).  None until a capture exists."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
         with open(p) as fh:
-            return json.load(fh).get(kernel)
+            for ln in fh.read().splitlines()[1:]:
+                name, val = ln.split(",")
+                if name == kernel:
+                    return int(val)
     except Exception:
-        return None
+        pass
+    return None
 
 
 def cpu_baseline(args, w):
