@@ -149,8 +149,9 @@ __device__ __forceinline__ uint32_t pack4(uint32_t v, uint32_t &inv4)
     const uint32_t ok = t3 & (~s7 & s6 & ~s3);
     uint32_t x = (v >> 1) & 0x03030303u;
     uint32_t c = x ^ ((x >> 1) & 0x01010101u);
-    inv4 = ((~ok & 0x01010101u) * 0x10204080u) >> 28; // bit j = symbol j invalid
-    return (c * 0x40100401u) >> 24;
+    // gathers as byte dot products (IDP.4A): bit j of inv4 = symbol j invalid; first symbol in the top two bits of the code byte
+    inv4 = __dp4a(~ok & 0x01010101u, 0x08040201u, 0u);
+    return __dp4a(c, 0x01041040u, 0u);
 }
 
 #ifdef SBF_DEFINE_AUX_KERNELS // non-template kernels: defined in one translation unit (sbf_api.cu)
