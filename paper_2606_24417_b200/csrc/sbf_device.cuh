@@ -138,19 +138,18 @@ __device__ __forceinline__ void red_or_64(uint64_t *p, uint64_t v)
 // =============================================================================================
 __device__ __forceinline__ uint32_t pack4(uint32_t v, uint32_t &inv4)
 {
-    // four ASCII bytes (first symbol in the low byte) -> 8 bits, first symbol in the top 2 bits
-    // validity as a boolean function of the bit planes (bit 0 of every byte of v >> j is bit j of that symbol;
-    // bit 5, the case bit, is ignored): A 0x41, C 0x43, G 0x47, T 0x54 <=> !b7 & b6 & !b3 &
-    // (b4 ? (b2 & !b1 & !b0) : (b0 & (b1 | !b2))).  Six shifts and five LOP3 for four symbols.
-    const uint32_t s1 = v >> 1, s2 = v >> 2, s3 = v >> 3, s4 = v >> 4, s6 = v >> 6, s7 = v >> 7;
-    const uint32_t t1 = v & (s1 | ~s2);
-    const uint32_t t2 = s2 & ~s1 & ~v;
-    const uint32_t t3 = (s4 & t2) | (~s4 & t1);
-    const uint32_t ok = t3 & (~s7 & s6 & ~s3);
-    uint32_t x = (v >> 1) & 0x03030303u;
-    uint32_t c = x ^ ((x >> 1) & 0x01010101u);
-    // gathers as byte dot products (IDP.4A): bit j of inv4 = symbol j invalid; first symbol in the top two bits of the code byte
-    inv4 = __dp4a(~ok & 0x01010101u, 0x08040201u, 0u);
+    // four ASCII bytes (first symbol in the low byte) -> 8 bits, first symbol in the top 2 bits.
+    // code = bits (b2, b1^b2) of the symbol: A 0, C 1, G 2, T 3 (either case).  Validity by the round trip: the
+    // symbol is valid iff, with its case bit cleared, it EQUALS the letter of its own code — one byte permute
+    // (PRMT as a 4-entry table "ACGT" indexed by the four codes) and one XOR instead of per-letter compares.
+    // The gathers are byte dot products (IDP.4A), which run off the alu pipe this kernel is bound by.
+    const uint32_t x = (v >> 1) & 0x03030303u;
+    const uint32_t c = x ^ ((x >> 1) & 0x01010101u);
+    const uint32_t sel = __dp4a(c, 0x00001001u, 0u) + (__dp4a(c, 0x10010000u, 0u) << 8); // the four codes as nibbles
+    const uint32_t diff = (v & 0xDFDFDFDFu) ^ __byte_perm(0x54474341u, 0u, sel);
+    // bit 7 of every byte of nz = that byte of diff is non-zero (no carry crosses a byte: 0x7F + 0x7F < 0x100)
+    const uint32_t nz = (((diff & 0x7F7F7F7Fu) + 0x7F7F7F7Fu) | diff) & 0x80808080u;
+    inv4 = __dp4a(nz, 0x08040201u, 0u) >> 7; // bit j = symbol j invalid
     return __dp4a(c, 0x01041040u, 0u);
 }
 
