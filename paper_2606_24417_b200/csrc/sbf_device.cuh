@@ -27,6 +27,9 @@
 #ifndef SBF_Q_PF
 #define SBF_Q_PF 3   // query (chunk mode): 0 load at first use, 1 prefetch.global.L2 ahead, 3 cp.async staging in shared memory
 #endif
+#ifndef SBF_IDP_EXTRACT
+#define SBF_IDP_EXTRACT 1 // bit-slice extraction by IDP.4A where the slice is byte aligned (H = 1, 2, 4, 8)
+#endif
 #ifndef SBF_MINB_I
 #define SBF_MINB_I 5 // insert: CTAs per SM the register budget is cut for (5 x 128 threads -> 96 registers)
 #endif
@@ -302,6 +305,15 @@ struct SlidingMin {
 template <int OFF>
 __device__ __forceinline__ uint64_t onehot_at(uint64_t h)
 {
+#if SBF_IDP_EXTRACT
+    if constexpr (OFF % 8 == 0) {
+        // byte-aligned slice: mask all four bytes of the half at once (shared by the other slices of that half), then
+        // pick the byte with a byte dot product (IDP.4A runs off the alu pipe that bounds the query kernels)
+        const uint32_t half = OFF < 32 ? (uint32_t)h : (uint32_t)(h >> 32);
+        const uint32_t b = __dp4a(half & 0x3F3F3F3Fu, 1u << (OFF % 32), 0u);
+        return 1ull << b;
+    }
+#endif
     return 1ull << ((h >> OFF) & 63);
 }
 
