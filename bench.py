@@ -39,6 +39,10 @@ METRIC = "G k-mers/s insert+query (1 step = insert the sequence + query one read
 OPS_PER_KMER = {"insert": 70.0, "query": 63.0}          # integer lane-ops
 # ALU peak derived in DESIGN.md §6: 148 SMs x 4 SMSPs x 16 lanes/clk (alu pipe, rt=2) x max SM clock
 ALU_LANES_PER_CLK = 148 * 4 * 16
+# measured on this pool's B200 with paper_2606_24417_b200/sbf_ceilings (profiles/ceilings_r01.txt): random 32-byte sector
+# accesses over a 512 MiB array, G accesses per second
+RANDOM_RMW_CEILING_G = 24.8   # one red.or.b64 per random sector (read + write-back)
+RANDOM_LD_CEILING_G = 50.0    # one 256-bit load per random sector
 
 
 def env_int(name, default):
@@ -442,6 +446,15 @@ def run_cuda(args):
                              "hbm_gbs_algorithmic": q_bytes / (qk * 1e-3) / 1e9},
             "pack_kernel_ms_mean": statistics.mean(pack_ms), "count_kernel_ms_mean": statistics.mean(count_ms),
         }
+        # random 32-byte sector accesses against the box's measured ceilings for them (profiles/ceilings_r01.txt,
+        # DESIGN.md §6): one read-modify-write per insert run (25 G/s), one 256-bit load per query run (50 G/s);
+        # runs estimated as k-mers x 2/(w+1) (+ one per record for the reads)
+        roof["insert_kernel"]["random_sector"] = {
+            "achieved_g_per_s": n_ins_kmers * d_runs / (ik * 1e-3) / 1e9, "ceiling_g_per_s": RANDOM_RMW_CEILING_G,
+            "frac": n_ins_kmers * d_runs / (ik * 1e-3) / 1e9 / RANDOM_RMW_CEILING_G}
+        roof["query_kernel"]["random_sector"] = {
+            "achieved_g_per_s": qk_kmers * (d_runs + 1.0 / per_read) / (qk * 1e-3) / 1e9, "ceiling_g_per_s": RANDOM_LD_CEILING_G,
+            "frac": qk_kmers * (d_runs + 1.0 / per_read) / (qk * 1e-3) / 1e9 / RANDOM_LD_CEILING_G}
         for kk in ("insert_kernel", "query_kernel"):
             roof[kk]["frac"] = roof[kk]["achieved"] / roof[kk]["peak"]
             roof[kk]["hbm_frac"] = roof[kk]["hbm_gbs_algorithmic"] / hbm_gbs
