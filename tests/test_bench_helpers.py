@@ -32,3 +32,14 @@ def test_reference_arm_line_has_the_contract_keys(capsys):
                 "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
         assert key in line
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle" and line["value"] > 0
+
+
+def test_sweep_helpers():
+    from paper_2606_24417_b200 import sweep
+    seq = np.frombuffer(b"ACGTNACGTACGTAC", dtype=np.uint8)
+    assert sweep._valid_windows(seq, 4) == 1 + 7           # ACGT | ACGTACGTAC has 7 windows of 4
+    reads = np.frombuffer(b"ACGTACGT" + b"ACNTACGT", dtype=np.uint8)
+    assert list(sweep._valid_per_read(reads, 8, 3)) == [6, 3]
+    pts = [dict(fpr_random=1e-3, time_ms=2.0), dict(fpr_random=1e-4, time_ms=3.0), dict(fpr_random=1e-3, time_ms=2.5),
+           dict(fpr_random=1e-5, time_ms=3.0)]
+    assert sweep.pareto(pts) == [0, 3]                     # 2 is dominated by 0, 1 by 3
