@@ -35,14 +35,12 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "G k-mers/s insert+query (1 step = insert the sequence + query one read batch)"
-# algorithmic work per valid k-mer, defaults k=31 m=16 s=28 H=4
-OPS_PER_KMER = {"insert": 70.0, "query": 63.0}          # integer lane-ops
-# ALU peak derived in DESIGN.md §6: 148 SMs x 4 SMSPs x 16 lanes/clk (alu pipe, rt=2) x max SM clock
-ALU_LANES_PER_CLK = 148 * 4 * 16
-# measured on this pool's B200 with paper_2606_24417_b200/sbf_ceilings (profiles/ceilings_r01.txt): random 32-byte sector
-# accesses over a 512 MiB array, G accesses per second
-RANDOM_RMW_CEILING_G = 24.8   # one red.or.b64 per random sector (read + write-back)
-RANDOM_LD_CEILING_G = 50.0    # one 256-bit load per random sector
+# ALGORITHMIC integer instructions per valid k-mer (defaults k=31 m=16 s=28 H=4), split by the
+# pipe they issue on: the multiplies of g, sigma and f (1 + 3 + 3 IMAD-class) go to the fma pipe, the rest to the alu pipe.
+OPS_PER_KMER = {"insert": {"alu": 63.0, "fma": 7.0}, "query": {"alu": 56.0, "fma": 7.0}}
+N_SMSP = 148 * 4
+# What the kernels EXECUTE (warp instructions per launch, by pipe): ncu counters of a committed capture, static.
+PIPES_CSV = os.path.join("profiles", "pipes_r02.csv")
 
 
 def env_int(name, default):
@@ -196,12 +194,13 @@ class ClockSampler:
 # ------------------------------------------------------------------------------------------------
 def oracle_sample_step(o, seq_sample, reads_sample, offs_sample, threads: bool):
     """One oracle 'step' on the bounded sample: clear, insert, query.  Returns (k-mers, seconds)."""
+    o.clear()                                   # the 512 MiB memset is not part of the oracle's insert rate
     t0 = time.perf_counter()
-    o.clear()
     n_ins = o.insert_records(seq_sample, threads=threads)
     t1 = time.perf_counter()
-    _, _, n_q = o.query_records(reads_sample, offs_sample, want_counts=True, threads=threads)
+    _, counts, n_q = o.query_records(reads_sample, offs_sample, want_counts=True, threads=threads)
     t2 = time.perf_counter()
+    oracle_sample_step.last_counts = counts
     return n_ins, n_q, t1 - t0, t2 - t1
 
 
@@ -373,6 +372,8 @@ def run_cuda(args):
         q_kernel_ms.append((mn, n_q_kmers[b])); pack_ms.append(pk); count_ms.append(ct)
     torch.cuda.synchronize()
 
+    ceilings = measure_ceilings(sbf, num_bits // 8) if rank == 0 else None
+
     # measured statistics of the last query batch: FPR on the uniform reads (odd read index)
     cnt = d_counts.cpu().numpy().view(np.uint32).astype(np.int64)
     per_read = max(w.read_len - k + 1, 1)
@@ -409,6 +410,20 @@ def run_cuda(args):
     e2e_s = time.perf_counter() - t0
     h2d = seq_h.numel() + n_read_bases + offs_np.nbytes
     d2h = hb_np.nbytes + hc_np.nbytes
+    # the host-facing calls must have produced what the device-facing calls produce on the same batch
+    e2e_filter = sbf.sbf_export_bits(h) if world == 1 else None
+    sbf.sbf_clear(h, stream)
+    do_insert(stream)
+    if world > 1:
+        replicas.or_allreduce_filter(h, stream=stream)
+    sbf.sbf_query_records(h, d_reads[b], d_offs, rb, n_read_bases, d_bitmap, d_counts, stream)
+    torch.cuda.synchronize()
+    e2e_ok = bool(np.array_equal(d_bitmap.cpu().numpy().view(np.uint32), hb_np)
+                  and np.array_equal(d_counts.cpu().numpy().view(np.uint32), hc_np)
+                  and (e2e_filter is None or np.array_equal(sbf.sbf_export_bits(h), e2e_filter)))
+    del e2e_filter
+    if not e2e_ok:
+        raise SystemExit("bench.py: the host-facing calls and the device-facing calls disagree on the same batch")
 
     # ---- reduce over ranks ------------------------------------------------------------------------
     kmers_local = args.steps * n_ins_kmers + q_total
@@ -427,47 +442,54 @@ def run_cuda(args):
         value = kmers_all / (total_ms * 1e-3) / 1e9
         ins_rate = ins_all / (ins_ms * 1e-3) / 1e9
         q_rate = q_all / (qry_ms * 1e-3) / 1e9
-        # rooflines.  ALU: algorithmic lane-ops / kernel time vs the alu-pipe peak at max clock.
-        alu_peak = ALU_LANES_PER_CLK * sm_max_mhz * 1e6 / 1e12          # T lane-ops/s
+        # ---- rooflines, against ceilings measured in this run ---------------------------------
         ik = statistics.mean(ins_kernel_ms)
         qk = statistics.mean(m for m, _ in q_kernel_ms)
         qk_kmers = statistics.mean(n for _, n in q_kernel_ms)
         w_ = k - p["m"] + 1
-        d_runs = 2.0 / (w_ + 1)
+        d_runs = 2.0 / (w_ + 1)                      # runs per k-mer on random sequence
+        clock_mhz = sm_max_mhz                       # rooflines are quoted at the maximum SM clock
+        ex_i, ex_i_src = load_pipes("insert_kernel")
+        ex_q, ex_q_src = load_pipes("query_kernel")
+        roof = {"insert_kernel": alu_roofline(OPS_PER_KMER["insert"], n_ins_kmers, ik, ceilings, clock_mhz, ex_i),
+                "query_kernel": alu_roofline(OPS_PER_KMER["query"], qk_kmers, qk, ceilings, clock_mhz, ex_q),
+                "pack_kernel_ms_mean": statistics.mean(pack_ms), "count_kernel_ms_mean": statistics.mean(count_ms)}
+        roof["insert_kernel"]["executed_source"], roof["query_kernel"]["executed_source"] = ex_i_src, ex_q_src
         # HBM: algorithmic bytes of the fused kernels (packed 2-bit words + mask + one sector read/write per run)
         ins_bytes = d_seq.numel() * (0.25 + 0.125) + n_ins_kmers * d_runs * 64.0
         q_bytes = n_read_bases * (0.25 + 0.125 + 0.125) + qk_kmers * (d_runs + 1.0 / per_read) * 32.0
-        roof = {
-            "insert_kernel": {"bound": "alu", "achieved": OPS_PER_KMER["insert"] * n_ins_kmers / (ik * 1e-3) / 1e12,
-                              "peak": alu_peak, "unit": "Tiop/s", "ms": ik, "gkmers_s": n_ins_kmers / ik / 1e6,
-                              "hbm_gbs_algorithmic": ins_bytes / (ik * 1e-3) / 1e9},
-            "query_kernel": {"bound": "alu", "achieved": OPS_PER_KMER["query"] * qk_kmers / (qk * 1e-3) / 1e12,
-                             "peak": alu_peak, "unit": "Tiop/s", "ms": qk, "gkmers_s": qk_kmers / qk / 1e6,
-                             "hbm_gbs_algorithmic": q_bytes / (qk * 1e-3) / 1e9},
-            "pack_kernel_ms_mean": statistics.mean(pack_ms), "count_kernel_ms_mean": statistics.mean(count_ms),
-        }
-        # random 32-byte sector accesses against the box's measured ceilings for them (profiles/ceilings_r01.txt,
-        # DESIGN.md §6): one read-modify-write per insert run (25 G/s), one 256-bit load per query run (50 G/s);
-        # runs estimated as k-mers x 2/(w+1) (+ one per record for the reads)
-        roof["insert_kernel"]["random_sector"] = {
-            "achieved_g_per_s": n_ins_kmers * d_runs / (ik * 1e-3) / 1e9, "ceiling_g_per_s": RANDOM_RMW_CEILING_G,
-            "frac": n_ins_kmers * d_runs / (ik * 1e-3) / 1e9 / RANDOM_RMW_CEILING_G}
-        roof["query_kernel"]["random_sector"] = {
-            "achieved_g_per_s": qk_kmers * (d_runs + 1.0 / per_read) / (qk * 1e-3) / 1e9, "ceiling_g_per_s": RANDOM_LD_CEILING_G,
-            "frac": qk_kmers * (d_runs + 1.0 / per_read) / (qk * 1e-3) / 1e9 / RANDOM_LD_CEILING_G}
-        for kk in ("insert_kernel", "query_kernel"):
-            roof[kk]["frac"] = roof[kk]["achieved"] / roof[kk]["peak"]
-            roof[kk]["hbm_frac"] = roof[kk]["hbm_gbs_algorithmic"] / hbm_gbs
+        for kk, nbytes, ms_ in (("insert_kernel", ins_bytes, ik), ("query_kernel", q_bytes, qk)):
+            roof[kk]["hbm"] = {"achieved": nbytes / (ms_ * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+                               "frac": nbytes / (ms_ * 1e-3) / 1e9 / hbm_gbs,
+                               "peak_source": peak_src + " (MEASURED_PEAKS.json hbm_gbs)"}
             if clocks.get("sm_mhz"):
-                roof[kk]["frac_at_achieved_clock"] = roof[kk]["achieved"] / (ALU_LANES_PER_CLK * clocks["sm_mhz"] * 1e6 / 1e12)
+                roof[kk]["frac_at_achieved_clock"] = roof[kk]["frac"] * clock_mhz / clocks["sm_mhz"]
+        # random 32-byte-sector accesses against the ceilings measured above for exactly that access: one
+        # read-modify-write (4 x RED.OR.B64) per insert run, one staged 2 x 16-byte cp.async per query run;
+        # runs = k-mers x 2/(w+1) (+ one per record for the reads)
+        rs = ceilings["random_sector_g_per_s"]
+        ins_runs_g = n_ins_kmers * d_runs / (ik * 1e-3) / 1e9
+        q_runs_g = qk_kmers * (d_runs + 1.0 / per_read) / (qk * 1e-3) / 1e9
+        rmw_ceiling = max(x for x in (rs.get("red_or_b64_x4"), rs.get("red_or_b64_x1")) if x)  # the better of the two
+        roof["insert_kernel"]["random_sector"] = {
+            "achieved_g_per_s": ins_runs_g, "ceiling_g_per_s": rmw_ceiling, "frac": ins_runs_g / rmw_ceiling,
+            "ceiling": "random red.or.b64 sectors/s over %d MiB, best of 1 and 4 RED per sector" % (num_bits >> 23)}
+        roof["query_kernel"]["random_sector"] = {
+            "achieved_g_per_s": q_runs_g, "ceiling_g_per_s": rs["cp_async_2x16"], "frac": q_runs_g / rs["cp_async_2x16"],
+            "ceiling": "random 2 x 16-byte cp.async sectors/s over %d MiB" % (num_bits >> 23)}
+        for kk in ("insert_kernel", "query_kernel"):  # which limit binds this kernel: instructions or random sectors
+            r = roof[kk]
+            busy = dict(r.get("busy_fraction_of_measured_limit", {"alu_pipe": r["frac"]}))
+            busy["random_sector"] = r["random_sector"]["frac"]
+            busy["hbm_bytes"] = r["hbm"]["frac"]
+            r["binds"] = max(busy, key=busy.get)
+            r["binds_busy"] = busy[r["binds"]]
         dom = "query_kernel" if qk * 1.0 >= ik else "insert_kernel"
-        traffic = load_traffic(dom)
-        roofline = {"bound": "alu", "kernel": dom, "achieved": roof[dom]["achieved"], "peak": alu_peak,
-                    "unit": "Tiop/s", "frac": roof[dom]["frac"], "traffic": traffic,
-                    "peak_source": "derived: 148 SM x 64 int lanes/clk x %.0f MHz (%s sm_max_mhz), DESIGN.md §6" % (
-                        sm_max_mhz, peak_src),
-                    "hbm": {"achieved": roof[dom]["hbm_gbs_algorithmic"], "peak": hbm_gbs, "unit": "GB/s",
-                            "frac": roof[dom]["hbm_frac"], "peak_source": peak_src + " (MEASURED_PEAKS.json hbm_gbs)"}}
+        traffic, traffic_src = load_traffic(dom)
+        roofline = {"bound": "alu", "kernel": dom, "achieved": roof[dom]["achieved"], "peak": roof[dom]["peak"],
+                    "unit": "Tiop/s", "frac": roof[dom]["frac"], "traffic": traffic, "traffic_source": traffic_src,
+                    "peak_source": roof[dom]["peak_source"], "binds": roof[dom]["binds"],
+                    "hbm": roof[dom]["hbm"]}
         line = {
             "metric": METRIC,
             "value": value, "unit": "G k-mers/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -485,12 +507,29 @@ def run_cuda(args):
             "clocks": clocks,
             "e2e": {"value": e2e_kmers_all / e2e_s / 1e9, "unit": "G k-mers/s", "h2d_bytes_per_step": int(h2d),
                     "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
-                    "api": "sbf_insert_seq_host + sbf_query_records_host (pinned host buffers)"},
+                    "api": "sbf_insert_seq_host + sbf_query_records_host (pinned host buffers)",
+                    "verified": "filter bytes, bitmap and hit counts equal the device-facing calls' on the same batch"},
             "gpu_launches": int(launches),
-            "roofline": roofline, "rooflines": roof,
+            "roofline": roofline, "rooflines": roof, "ceilings": ceilings,
         }
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline(args, w)
+            line["cpu_baseline"], sample, o_counts = cpu_baseline(args, w)
+            # the same bounded sample through the CUDA path: the two FPRs are one statistic (equal by parity)
+            seq_s, reads_s, offs_s = sample
+            h2 = sbf.sbf_create(k, p["m"], p["s"], p["H"], p["num_bits"])
+            sbf.sbf_insert_seq(h2, torch.from_numpy(seq_s).cuda(), seq_s.size)
+            bm2 = torch.empty((reads_s.size + 31) // 32, dtype=torch.int32, device="cuda")
+            hc2 = torch.empty(offs_s.size - 1, dtype=torch.int32, device="cuda")
+            sbf.sbf_query_records(h2, torch.from_numpy(reads_s).cuda(), torch.from_numpy(offs_s.view(np.int64)).cuda(),
+                                  offs_s.size - 1, reads_s.size, bm2, hc2)
+            torch.cuda.synchronize()
+            g_counts = hc2.cpu().numpy().view(np.uint32)
+            sbf.sbf_destroy(h2)
+            n_alien = max(1, g_counts[1::2].size * per_read)
+            line["fpr"]["same_sample"] = {
+                "sample": line["cpu_baseline"]["sample"], "gpu": float(g_counts[1::2].astype(np.int64).sum()) / n_alien,
+                "oracle": float(o_counts[1::2].astype(np.int64).sum()) / n_alien,
+                "hit_counts_identical": bool(np.array_equal(g_counts, o_counts))}
         print(json.dumps(line))
     sbf.sbf_destroy(h)
     if world > 1:
@@ -498,20 +537,81 @@ def run_cuda(args):
     return 0
 
 
-def load_traffic(kernel: str):
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture
-    (profiles/traffic.csv, written from the .ncu-rep's dram__bytes_read.sum + dram__bytes_write.sum; see
-    profiles/ncu_full_r01.md).  None until a capture exists."""
-    p = os.path.join(ROOT, "profiles", "traffic.csv")
+def load_csv_rows(rel):
     try:
-        with open(p) as fh:
-            for ln in fh.read().splitlines()[1:]:
-                name, val = ln.split(",")
-                if name == kernel:
-                    return int(val)
+        with open(os.path.join(ROOT, rel)) as fh:
+            lines = [ln for ln in fh.read().splitlines() if ln and not ln.startswith("#")]
+        hdr = lines[0].split(",")
+        return [dict(zip(hdr, ln.split(","))) for ln in lines[1:]]
     except Exception:
-        pass
-    return None
+        return []
+
+
+def load_traffic(kernel: str):
+    """DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum of a committed
+    `ncu --set full` capture, profiles/traffic.csv).  STATIC: it describes the build that was profiled, which the
+    `source` column names; None until a capture exists."""
+    for r in load_csv_rows(os.path.join("profiles", "traffic.csv")):
+        if r.get("kernel") == kernel:
+            return int(r["dram_bytes_per_launch"]), r.get("source", "profiles/traffic.csv")
+    return None, None
+
+
+def load_pipes(kernel: str):
+    """Executed warp instructions per launch by pipe (ncu smsp__inst_executed_pipe_*.sum; static, see PIPES_CSV)."""
+    for r in load_csv_rows(PIPES_CSV):
+        if r.get("kernel") == kernel:
+            return {k: float(v) for k, v in r.items() if k not in ("kernel", "source")}, r.get("source", PIPES_CSV)
+    return None, None
+
+
+def measure_ceilings(sbf, filter_bytes):
+    """The box's ceilings, measured in THIS run through the library's sbf_ceiling_* entry points: issue rates of
+    one SM sub-partition by instruction mix (warp instructions per clock, counted in SASS) and random 32-byte-sector
+    access rates over an array as large as the filter."""
+    pipes, clk = {}, []
+    for mode in range(sbf.sbf_ceiling_pipe_modes()):
+        r, c = sbf.sbf_ceiling_pipe_rate(mode, 2048)
+        pipes[sbf.sbf_ceiling_pipe_mode_name(mode)] = r
+        clk.append(c)
+    names = ["red_or_b64_x4", "red_or_b64_x1", "ld_nc_256", "cp_async_2x16", "tma_reduce_or_32B"]
+    rnd = {}
+    for mode, nm in enumerate(names):
+        try:
+            rnd[nm] = sbf.sbf_ceiling_random_sector(mode, min(filter_bytes, 8 << 30))
+        except Exception as e:  # noqa: BLE001 - a ceiling that cannot be measured is reported as such
+            rnd[nm] = None
+    return {"source": "measured in this run (sbf_ceiling_pipe_rate / sbf_ceiling_random_sector, include/sbf.h)",
+            "pipe_warp_inst_per_clk_per_smsp": pipes, "sm_clock_mhz_during_pipe_runs": statistics.median(clk),
+            "random_sector_g_per_s": rnd, "random_sector_array_bytes": int(min(filter_bytes, 8 << 30))}
+
+
+def alu_roofline(ops, n_units, ms, ceil, clock_mhz, executed):
+    """Instruction roofline of one kernel.  achieved = ALGORITHMIC lane-ops per second.  peak = the rate the SM
+    sub-partitions can issue that algorithmic mix at: per unit the alu-pipe ops need ops_alu / r_alu clocks, the
+    fma-pipe ops ops_fma / r_fma, and all of them together (ops_alu + ops_fma) / r_issue; the slowest binds
+    (r_* measured: pure LOP3, pure IMAD, LOP3:IMAD 1:1).  `executed` (ncu) gives the same three times for the
+    instructions the kernel really issues: their ratio to the kernel's duration is how busy each limit is."""
+    pr = ceil["pipe_warp_inst_per_clk_per_smsp"]
+    r_alu, r_fma, r_issue = pr["LOP3"], pr["IMAD"], pr["LOP3:IMAD 1:1"]
+    total = ops["alu"] + ops["fma"]
+    clk_per_unit = max(ops["alu"] / r_alu, ops["fma"] / r_fma, total / r_issue)   # per warp of 32 units, per SMSP
+    lanes_per_s = 32.0 * N_SMSP * clock_mhz * 1e6
+    peak = total / clk_per_unit * lanes_per_s / 1e12                                # T lane-ops/s for this mix
+    achieved = total * n_units / (ms * 1e-3) / 1e12
+    out = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tiop/s", "frac": achieved / peak, "ms": ms,
+           "gkmers_s": n_units / ms / 1e6,
+           "algorithmic_ops_per_kmer": dict(ops), "peak_source": "measured: pipe rates alu %.3f fma %.3f issue %.3f "
+           "warp-inst/clk/SMSP x %d SMSP x %.0f MHz" % (r_alu, r_fma, r_issue, N_SMSP, clock_mhz)}
+    if executed:
+        cyc = ms * 1e-3 * clock_mhz * 1e6 * N_SMSP                                   # SMSP-cycles of the launch
+        busy = {"alu_pipe": executed["inst_alu"] / r_alu / cyc, "fma_pipe": executed["inst_fma"] / r_fma / cyc,
+                "issue": executed["inst_total"] / r_issue / cyc}
+        out["executed_warp_inst_per_kmer"] = {k[5:]: v * 32.0 / executed["units"] for k, v in executed.items()
+                                              if k.startswith("inst_")}
+        out["busy_fraction_of_measured_limit"] = busy
+        out["binding_instruction_limit"] = max(busy, key=busy.get)
+    return out
 
 
 def cpu_baseline(args, w):
@@ -527,9 +627,10 @@ def cpu_baseline(args, w):
     single = {"value": (a + b) / (ti + tq) / 1e9, "insert": a / ti / 1e9, "query": b / tq / 1e9}
     a, b, ti, tq = oracle_sample_step(o, seq_s, reads_s, offs_s, True)
     cores = oracle.num_threads()
-    return {"value": (a + b) / (ti + tq) / 1e9, "unit": "G k-mers/s", "cores": cores, "kind": "oracle",
-            "sample": sample, "insert_gkmers_s": a / ti / 1e9, "query_gkmers_s": b / tq / 1e9,
-            "single_thread": single}
+    return ({"value": (a + b) / (ti + tq) / 1e9, "unit": "G k-mers/s", "cores": cores, "kind": "oracle",
+             "sample": sample, "insert_gkmers_s": a / ti / 1e9, "query_gkmers_s": b / tq / 1e9,
+             "timed": "insert + query of the sample (the filter is cleared before the clock starts)",
+             "single_thread": single}, (seq_s, reads_s, offs_s), oracle_sample_step.last_counts)
 
 
 def main():

@@ -130,6 +130,12 @@ int sbf_query_seq_host(sbf_t *f, const char *h_seq, uint64_t len, uint32_t *h_bi
 int sbf_query_records_host(sbf_t *f, const char *h_bases, const uint64_t *h_offsets, uint64_t n_rec,
                            uint32_t *h_bitmap, uint32_t *h_hit_counts);
 
+/* sbf_set_host_chunk — symbols per staged chunk of the host-facing calls ("multi-chunk workloads"):
+ * a multiple of 128, larger than k + 128; default 32 Mi (the measured optimum on B200 / PCIe 5).  Chunks overlap by
+ * k-1 symbols so that every k-mer lies wholly inside one chunk.  A tuning knob; tests use small chunks to put
+ * record boundaries before, on and inside the overlap. */
+int sbf_set_host_chunk(sbf_t *f, uint64_t symbols);
+
 /* sbf_export_bits — copy the filter (32*numShards bytes, layout A12) to host memory.
  * nbytes must equal 32*numShards.  Synchronises the device. */
 int sbf_export_bits(const sbf_t *f, void *h_dst, uint64_t nbytes);
@@ -161,6 +167,26 @@ uint64_t sbf_kernel_launches(void);
  * bench.py uses these for the per-kernel roofline figures. */
 int sbf_set_timing(sbf_t *f, int on);
 int sbf_get_timing(sbf_t *f, float *ms3);
+
+/*
+ * Measured ceilings of the device ("measure ... before quoting a denominator").  Not part of the
+ * path; bench.py calls them in the same run as the kernels it times and reports the rooflines against them.
+ *
+ * sbf_ceiling_pipe_rate — issue rate of one SM sub-partition for a fixed instruction mix, in warp instructions per
+ *   SM clock, counted in SASS (each loop body is N x one instruction; tests/test_ceilings_sass.py checks the
+ *   disassembly).  mode < sbf_ceiling_pipe_modes(); sbf_ceiling_pipe_mode_name(mode) names the mix, e.g. "LOP3"
+ *   (alu pipe), "IMAD" (fma pipe), "LOP3:IMAD 3:1".  iters = loop iterations of 256 instructions per warp.
+ *   *sm_clock_mhz (nullable) = loop cycles / kernel time, the SM clock during the run.
+ * sbf_ceiling_random_sector — random 32-byte-sector accesses per second (in 1e9/s) over a zeroed scratch array of
+ *   array_bytes (rounded down to a power of two), allocated and freed inside the call.  mode 0: 4 x red.or.b64 per
+ *   sector (the insert kernel's flush), 1: 1 x red.or.b64, 2: one 256-bit ld.global.nc, 3: 2 x 16-byte cp.async into
+ *   shared memory (the query kernels' staging), 4: one 32-byte cp.reduce.async.bulk .or.b64 (TMA reduction).
+ * Both synchronise the device.
+ */
+int sbf_ceiling_pipe_modes(void);
+const char *sbf_ceiling_pipe_mode_name(int mode);
+int sbf_ceiling_pipe_rate(int mode, int iters, double *warp_inst_per_clk_per_smsp, double *sm_clock_mhz);
+int sbf_ceiling_random_sector(int mode, uint64_t array_bytes, double *g_accesses_per_s);
 
 /* Diagnostics for tests: dump the internal 2-bit packed words / validity mask of the LAST batch
  * (device->host, synchronises).  n_words = ceil(bases/16); mask has one uint16 per word. */

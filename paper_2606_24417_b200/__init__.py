@@ -51,9 +51,14 @@ ABI = {
     "sbf_or_range_device": (_i32, [_p, _u64, _p, _u64, _p]),
     "sbf_last_error": (_cp, []),
     "sbf_kernel_launches": (_u64, []),
+    "sbf_set_host_chunk": (_i32, [_p, _u64]),
     "sbf_set_timing": (_i32, [_p, _i32]),
     "sbf_get_timing": (_i32, [_p, _p]),
     "sbf_debug_last_packed": (_i32, [_p, _p, _p, _u64]),
+    "sbf_ceiling_pipe_modes": (_i32, []),
+    "sbf_ceiling_pipe_mode_name": (_cp, [_i32]),
+    "sbf_ceiling_pipe_rate": (_i32, [_i32, _i32, _p, _p]),
+    "sbf_ceiling_random_sector": (_i32, [_i32, _u64, _p]),
 }
 
 
@@ -64,15 +69,19 @@ class SBFError(RuntimeError):
 
 
 def load_library(build_if_missing: bool = True):
-    """dlopen libsbf_b200.so (building it with nvcc first if it is not there) and type every symbol."""
+    """dlopen libsbf_b200.so and type every symbol.  With build_if_missing the (mtime-incremental) build runs
+    first, so a library older than its sources is never loaded; without nvcc an existing library is used as is."""
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH):
-        if not build_if_missing:
-            raise SBFError(SBF_ERR_UNSUPPORTED, "libsbf_b200.so not built (python -m paper_2606_24417_b200.build)")
+    if build_if_missing and LIB_PATH == os.path.join(_HERE, "libsbf_b200.so"):
         from . import build as _build
-        _build.build()
+        try:
+            _build.build()
+        except FileNotFoundError:          # no nvcc on this box: fall through to whatever was shipped
+            pass
+    if not os.path.exists(LIB_PATH):
+        raise SBFError(SBF_ERR_UNSUPPORTED, "libsbf_b200.so not built (python -m paper_2606_24417_b200.build)")
     L = ctypes.CDLL(LIB_PATH)
     for name, (res, args) in ABI.items():
         fn = getattr(L, name)  # AttributeError here = the library does not export what sbf.h declares
@@ -201,6 +210,10 @@ def sbf_or_range_device(h, offset_bytes: int, d_src, nbytes: int, stream=None):
     _check(load_library().sbf_or_range_device(h, offset_bytes, _dptr(d_src), nbytes, _stream(stream)))
 
 
+def sbf_set_host_chunk(h, symbols: int):
+    _check(load_library().sbf_set_host_chunk(h, symbols))
+
+
 def sbf_set_timing(h, on: bool):
     _check(load_library().sbf_set_timing(h, 1 if on else 0))
 
@@ -210,6 +223,24 @@ def sbf_get_timing(h):
     ms = (ctypes.c_float * 3)()
     _check(load_library().sbf_get_timing(h, ctypes.cast(ms, ctypes.c_void_p)))
     return float(ms[0]), float(ms[1]), float(ms[2])
+
+
+def sbf_ceiling_pipe_modes() -> int: return int(load_library().sbf_ceiling_pipe_modes())
+def sbf_ceiling_pipe_mode_name(mode: int) -> str: return load_library().sbf_ceiling_pipe_mode_name(mode).decode()
+
+
+def sbf_ceiling_pipe_rate(mode: int, iters: int = 2048):
+    """(warp instructions per clock per SM sub-partition, SM clock in MHz) of one instruction mix."""
+    r, c = ctypes.c_double(0), ctypes.c_double(0)
+    _check(load_library().sbf_ceiling_pipe_rate(mode, iters, ctypes.addressof(r), ctypes.addressof(c)))
+    return float(r.value), float(c.value)
+
+
+def sbf_ceiling_random_sector(mode: int, array_bytes: int) -> float:
+    """Random 32-byte-sector accesses per second (1e9/s) over array_bytes."""
+    g = ctypes.c_double(0)
+    _check(load_library().sbf_ceiling_random_sector(mode, array_bytes, ctypes.addressof(g)))
+    return float(g.value)
 
 
 def sbf_debug_last_packed(h, n_words: int):

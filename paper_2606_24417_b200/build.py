@@ -87,21 +87,5 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str =
     return lib
 
 
-TOOL = os.path.join(HERE, "sbf_ceilings")
-
-
-def build_tools(force: bool = False) -> str:
-    """csrc/tools/ceilings.cu -> paper_2606_24417_b200/sbf_ceilings (micro-benchmarks behind DESIGN.md §6)."""
-    src = os.path.join(CSRC, "tools", "ceilings.cu")
-    if force or not os.path.exists(TOOL) or os.path.getmtime(TOOL) < os.path.getmtime(src):
-        r = subprocess.run([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-std=c++17", "-O3", "-lineinfo",
-                            "-o", TOOL + ".tmp", src], stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
-        if r.returncode != 0:
-            raise RuntimeError("nvcc failed on ceilings.cu\n" + r.stdout)
-        os.replace(TOOL + ".tmp", TOOL)
-    return TOOL
-
-
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
-    print(build_tools(force="--force" in sys.argv))

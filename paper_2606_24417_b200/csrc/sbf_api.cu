@@ -18,6 +18,8 @@ using namespace sbfk;
 
 namespace {
 
+constexpr uint64_t kHostChunkDefault = 32ull << 20; // host-facing path: symbols per staged chunk, multiple of 128 (measured best of 8..128 Mi)
+
 thread_local std::string g_err;
 std::atomic<uint64_t> g_launches{0};
 
@@ -121,6 +123,7 @@ struct sbf {
     bool l2_stream_valid;
     // host-facing staging (created on first use)
     HostRun *host;
+    uint64_t host_chunk;      // symbols per staged chunk (sbf_set_host_chunk; default kHostChunkDefault)
     // optional per-kernel timing (sbf_set_timing): events on the caller's stream around each kernel
     bool timing;
     cudaEvent_t tev[4]; // before pack, after pack, after main kernel, after count kernel
@@ -352,6 +355,7 @@ sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits)
     }
     f->k = k; f->m = m; f->s = s; f->H = H; f->P = P; f->device = dev;
     f->num_shards = shards;
+    f->host_chunk = kHostChunkDefault;
     f->entry = find_entry(k, m, s, H);
     e = cudaMalloc(&f->filter, shards * 32);
     if (e == cudaSuccess) e = cudaMemset(f->filter, 0, shards * 32);
@@ -401,6 +405,15 @@ int sbf_reserve(sbf_t *f, uint64_t max_bases)
 {
     if (!f) return fail(SBF_ERR_INVALID_ARG, "sbf_reserve: NULL handle");
     return ensure_scratch(f, max_bases);
+}
+
+int sbf_set_host_chunk(sbf_t *f, uint64_t symbols)
+{
+    if (!f) return fail(SBF_ERR_INVALID_ARG, "sbf_set_host_chunk: NULL handle");
+    if (symbols == 0 || (symbols & 127) || symbols < 128 + (uint64_t)f->k)
+        return fail(SBF_ERR_INVALID_ARG, "sbf_set_host_chunk: need a multiple of 128 symbols, larger than k + 128");
+    f->host_chunk = symbols;
+    return SBF_OK;
 }
 
 int sbf_set_timing(sbf_t *f, int on)
@@ -540,7 +553,7 @@ int sbf_debug_last_packed(const sbf_t *f, uint32_t *h_words, uint16_t *h_mask, u
 
 // =============================================================================================
 // C ABI — host-facing ("host-facing calls synchronise"; staging after P:323-325):
-// the batch is cut in chunks of kHostChunk symbols that overlap by k-1, so that every k-mer
+// the batch is cut in chunks of host_chunk symbols (default 32 Mi) that overlap by k-1, so that every k-mer
 // start position belongs to exactly one chunk and is complete inside it.  A copy stream moves
 // chunk c+1 to the device while the compute stream packs and walks chunk c; results come back
 // chunk by chunk.  Pageable caller memory is staged through two pinned buffers; pinned or
@@ -548,7 +561,6 @@ int sbf_debug_last_packed(const sbf_t *f, uint32_t *h_words, uint16_t *h_mask, u
 // =============================================================================================
 namespace {
 
-constexpr uint64_t kHostChunk = 32ull << 20; // symbols per chunk, multiple of 128 (measured best of 8..128 Mi: DESIGN.md §6)
 
 bool is_pinned(const void *p)
 {
@@ -572,12 +584,13 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
     // the internal streams are non-blocking: order this call after everything the caller enqueued before it
     CK(cudaDeviceSynchronize());
     const uint64_t ov = (uint64_t)f->k - 1;
+    const uint64_t kHostChunk = f->host_chunk;
     const uint64_t span = (total < kHostChunk ? total : kHostChunk) + ov; // largest chunk incl. overlap
     const uint64_t n_chunks = (total + kHostChunk - 1) / kHostChunk;
     const bool direct = is_pinned(h_bases);
-    // most record boundaries a chunk can hold: all of them, bounded by its symbols (+2 ends)
-    uint64_t max_off = (n_rec + 2 < span + 2 ? n_rec + 2 : span + 2);
-    if (!h_offsets) max_off = 2;
+    // most record boundaries a chunk can hold: all of them (+2 ends).  Empty records repeat an offset, so the
+    // chunk's symbol count is NOT a bound.
+    const uint64_t max_off = h_offsets ? n_rec + 2 : 2;
 
     if (!f->host) {
         f->host = new (std::nothrow) HostRun();

@@ -583,6 +583,9 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
             }
         }
     }
+    // the last LA positions of a chunk staged look-ahead copies nobody reads; drain them before the next chunk's
+    // prologue reuses the same staging slots (two unordered cp.async to one slot could land in either order)
+    if constexpr (STAGE) cp_async_wait<0>();
     } // chunk loop
 }
 

@@ -115,7 +115,8 @@ def or_allreduce(local, or_into: Callable[[int, object], None], group=None, wind
         #     when they do, by one all_gather when they are equal)
         lens = {p1 - p0 for p0, p1 in sl}
         if len(lens) == 1 and my1 > my0:
-            dist.all_gather([local[a + p0:a + p1] for p0, p1 in sl], local[a + my0:a + my1].clone(), group=group)
+            # in place: this rank's input IS slot `rank` of the output (the layout NCCL's in-place all-gather wants)
+            dist.all_gather_into_tensor(local[a:a + w], local[a + my0:a + my1], group=group)
         else:
             for src in range(world):
                 p0, p1 = sl[src]
@@ -148,11 +149,25 @@ def filter_tensor(handle):
 
 
 def or_allreduce_filter(handle, group=None, stream=None, window_bytes: int = 1 << 28) -> int:
-    """The insert path's exchange step on GPUs: all-gather windows of the replicas over NCCL/NVLink,
-    OR them in with the library's kernel."""
+    """The insert path's exchange step on GPUs: per window of the filter a reduce-scatter (batched NCCL
+    point-to-point over NVLink + the library's OR kernel) and an in-place all-gather (see or_allreduce).
+
+    Ordering: NCCL collectives synchronise with torch's CURRENT stream only, so the whole exchange runs with
+    `stream` (the stream the inserts were enqueued on; None = the current one) made current: the sends then wait
+    for the inserts, every OR kernel waits for its receive, and the next window's receives wait for the ORs that
+    still read the scratch buffer."""
+    import torch
     from . import sbf_or_range_device
 
-    def or_into(offset: int, chunk):
-        sbf_or_range_device(handle, offset, chunk, chunk.numel(), stream)
+    if stream is None:
+        st = torch.cuda.current_stream()
+    elif isinstance(stream, int):
+        st = torch.cuda.ExternalStream(stream)
+    else:
+        st = stream
 
-    return or_allreduce(filter_tensor(handle), or_into, group=group, window_bytes=window_bytes)
+    def or_into(offset: int, chunk):
+        sbf_or_range_device(handle, offset, chunk, chunk.numel(), st)
+
+    with torch.cuda.stream(st):
+        return or_allreduce(filter_tensor(handle), or_into, group=group, window_bytes=window_bytes)

@@ -43,3 +43,31 @@ def test_sweep_helpers():
     pts = [dict(fpr_random=1e-3, time_ms=2.0), dict(fpr_random=1e-4, time_ms=3.0), dict(fpr_random=1e-3, time_ms=2.5),
            dict(fpr_random=1e-5, time_ms=3.0)]
     assert sweep.pareto(pts) == [0, 3]                     # 2 is dominated by 0, 1 by 3
+
+
+def test_instruction_roofline_model():
+    """alu_roofline: the peak is the measured issue rate of the ALGORITHMIC alu:fma mix; executed counts give busy fractions."""
+    ceil = {"pipe_warp_inst_per_clk_per_smsp": {"LOP3": 0.5, "IMAD": 0.5, "LOP3:IMAD 1:1": 1.0}}
+    ops = {"alu": 56.0, "fma": 7.0}
+    # 592 SMSPs at 1000 MHz; the alu pipe binds: 56 / 0.5 = 112 clocks per warp of 32 k-mers
+    n, ms = 32 * 592 * 1000, 1.0
+    r = bench.alu_roofline(ops, n, ms, ceil, 1000.0, None)
+    ideal_ms = 112 * 1000 / 1000e6 * 1e3
+    assert abs(r["frac"] - ideal_ms / ms) < 1e-9 and r["bound"] == "alu"
+    assert abs(r["peak"] - 63.0 / 112.0 * 32 * 592 * 1e9 / 1e12) < 1e-9
+    ex = {"units": float(n), "inst_total": 90.0 * n / 32, "inst_alu": 57.0 * n / 32, "inst_fma": 16.0 * n / 32}
+    r = bench.alu_roofline(ops, n, ms, ceil, 1000.0, ex)
+    cyc = 1e-3 * 1000e6 * 592
+    assert abs(r["busy_fraction_of_measured_limit"]["alu_pipe"] - (57.0 * n / 32) / 0.5 / cyc) < 1e-9
+    assert r["binding_instruction_limit"] == "alu_pipe"
+    assert abs(r["executed_warp_inst_per_kmer"]["alu"] - 57.0) < 1e-9
+    # an fma-heavy mix is bound by issue, not by either pipe
+    r = bench.alu_roofline({"alu": 30.0, "fma": 30.0}, n, ms, ceil, 1000.0, None)
+    assert abs(r["peak"] - 1.0 * 32 * 592 * 1e9 / 1e12) < 1e-9
+
+
+def test_static_profile_tables_load():
+    rows = bench.load_csv_rows("profiles/traffic.csv")
+    assert rows and {"kernel", "dram_bytes_per_launch", "source"} <= set(rows[0])
+    t, src = bench.load_traffic("query_kernel")
+    assert t > 0 and "ncu" in src

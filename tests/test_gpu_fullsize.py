@@ -27,8 +27,18 @@ def _first_diff(got, want, what):
                          (what, bad.size, got.size, bad[0], got[bad[0]], want[bad[0]]))
 
 
+_c3 = {}
+
+
+def _config3():
+    """The config-3 workload, generated once per session (250 Mbp, N runs)."""
+    if "w" not in _c3:
+        _c3["w"] = seqgen.config3()
+    return _c3["w"]
+
+
 def test_config3_full_size_filter_bitmap_counts():
-    w = seqgen.config3()                       # 250 Mbp, N runs, 2^32-bit filter
+    w = _config3()                             # 250 Mbp, N runs, 2^32-bit filter
     nb = w.params["num_bits"]
     n_reads = 4_000_000                        # bench.py's batch
     reads = w.read_batch(0, n_reads)
@@ -157,4 +167,120 @@ def test_config4_full_size_insert_and_query_batch():
         wbm, wc, _ = o.query_records(reads, offs, threads=True)
         _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "bitmap words")
         _first_diff(hc.cpu().numpy().view(np.uint32), wc, "hit counts")
+    o.close()
+
+
+def test_config3_chunk_mode_query_of_the_inserted_sequence():
+    """sbf_query_seq of long sequences runs the CHUNK-mode query kernel; its chunk length depends on the batch size
+    (chunk_blocks 8 from 64 Mi symbols, 4 from 16 Mi).  Config 1's "query the same sequence" at config-3 size: the
+    whole 250 Mbp sequence against its own 2^32-bit filter (chunk_blocks 8) and a 20 Mbp stretch (chunk_blocks 4);
+    bitmap equal to the oracle's and every valid k-mer true."""
+    w = _config3()
+    nb = w.params["num_bits"]
+    o = oracle.OracleSBF(num_bits=nb, **DEFAULT)
+    o.insert_records(w.insert_bases, threads=True)
+    with sbf.SuperBloomFilter(num_bits=nb, **DEFAULT) as f:
+        d_seq = _dev(w.insert_bases)
+        f.insert_seq(d_seq)
+        for a, n in ((0, w.insert_bases.size), (100_000_000, 20_000_000)):
+            assert n >= (64 << 20) or (16 << 20) <= n < (64 << 20)
+            view = d_seq[a:a + n]
+            bm = torch.full(((n + 31) // 32,), -1, dtype=torch.int32, device="cuda")
+            hits = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+            sbf.sbf_query_seq(f.handle, view, n, bm, hits)
+            torch.cuda.synchronize()
+            wbm, wc, n_valid = o.query_records(w.insert_bases[a:a + n], None, threads=True)
+            _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "chunk-mode bitmap words (n = %d)" % n)
+            assert int(hits.item()) == int(wc.sum()) == n_valid
+    o.close()
+
+
+def test_strided_chunk_fallback_behind_record_mode():
+    """A batch of 150-base reads plus ONE record above the record-mode limit hands the whole batch to the chunk-mode
+    query kernel, which then runs with a capped grid and STRIDES over several chunks per thread (> 4.85 M symbols):
+    the staging slots are reused from one chunk to the next."""
+    w = _config3()
+    n_reads = 60_000
+    reads = w.read_batch(0, n_reads)                               # 9 M symbols
+    lens = np.full(n_reads + 1, 150, dtype=np.int64)
+    lens[30_000] = 5000
+    offs = np.concatenate(([0], np.cumsum(lens))).astype(np.uint64)
+    q = np.empty(int(offs[-1]), dtype=np.uint8)
+    a = 30_000 * 150
+    q[:a] = reads[:a]
+    q[a:a + 5000] = w.insert_bases[1_000_000:1_005_000]
+    q[a + 5000:] = reads[a:]
+    ins = np.ascontiguousarray(w.insert_bases[:20_000_000])
+    o = oracle.OracleSBF(num_bits=1 << 30, **DEFAULT)
+    o.insert_records(ins, threads=True)
+    with sbf.SuperBloomFilter(num_bits=1 << 30, **DEFAULT) as f:
+        f.insert_seq(_dev(ins))
+        for rep in range(3):                                       # an ordering bug would be intermittent
+            bm = torch.full(((q.size + 31) // 32,), -1, dtype=torch.int32, device="cuda")
+            hc = torch.full((offs.size - 1,), -1, dtype=torch.int32, device="cuda")
+            f.query_records(_dev(q), _dev(offs.view(np.int64)), bm, hc)
+            torch.cuda.synchronize()
+            if rep == 0:
+                wbm, wc, _ = o.query_records(q, offs, threads=True)
+            _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "bitmap words")
+            _first_diff(hc.cpu().numpy().view(np.uint32), wc, "hit counts")
+    o.close()
+
+
+AXES = sorted({(s, 16, 4) for s in seqgen.SWEEP_S} | {(28, m, 4) for m in seqgen.SWEEP_M} | {(28, 16, h) for h in seqgen.SWEEP_H})
+
+
+@pytest.mark.parametrize("s,m,H", AXES)
+def test_config5_axes_at_full_config3_size(s, m, H):
+    """BASELINE config 5, the one-factor-at-a-time axes through (28,16,4) at FULL size: the whole
+    250 Mbp sequence into a 2^32-bit filter (every filter byte) and one batch of 10^6 reads (bitmap + counts)."""
+    w = _config3()
+    params = dict(k=31, m=m, s=s, H=H)
+    nb = w.params["num_bits"]
+    n_reads = 1_000_000
+    if "reads" not in _c3:
+        _c3["reads"] = w.read_batch(0, n_reads)
+    reads, offs = _c3["reads"], seqgen.fixed_offsets(n_reads, w.read_len)
+    o = oracle.OracleSBF(num_bits=nb, **params)
+    o.insert_records(w.insert_bases, threads=True)
+    with sbf.SuperBloomFilter(num_bits=nb, **params) as f:
+        assert f.specialized
+        f.insert_seq(_dev(w.insert_bases))
+        torch.cuda.synchronize()
+        _first_diff(f.export_bits(), o.export_bits(), "filter bytes %r" % (params,))
+        bm = torch.full(((reads.size + 31) // 32,), -1, dtype=torch.int32, device="cuda")
+        hc = torch.full((n_reads,), -1, dtype=torch.int32, device="cuda")
+        f.query_records(_dev(reads), _dev(offs.view(np.int64)), bm, hc)
+        torch.cuda.synchronize()
+        wbm, wc, _ = o.query_records(reads, offs, threads=True)
+        _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "bitmap words %r" % (params,))
+        _first_diff(hc.cpu().numpy().view(np.uint32), wc, "hit counts %r" % (params,))
+    o.close()
+
+
+@pytest.mark.parametrize("log2_bits", seqgen.SWEEP_LOG2_BITS)
+def test_config5_filter_sizes_at_full_config3_size(log2_bits):
+    """BASELINE config 5's seven filter sizes 2^28 .. 2^34 bits at (28,16,4): full sequence, one batch of 10^6 reads."""
+    if log2_bits == 32:
+        pytest.skip("2^32 bits is test_config3_full_size_filter_bitmap_counts")
+    w = _config3()
+    nb = 1 << log2_bits
+    n_reads = 1_000_000
+    if "reads" not in _c3:
+        _c3["reads"] = w.read_batch(0, n_reads)
+    reads, offs = _c3["reads"], seqgen.fixed_offsets(n_reads, w.read_len)
+    o = oracle.OracleSBF(num_bits=nb, **DEFAULT)
+    o.insert_records(w.insert_bases, threads=True)
+    with sbf.SuperBloomFilter(num_bits=nb, **DEFAULT) as f:
+        assert f.num_shards == o.num_shards == 1 << (log2_bits - 8)
+        f.insert_seq(_dev(w.insert_bases))
+        torch.cuda.synchronize()
+        _first_diff(f.export_bits(), o.words().reshape(-1).view(np.uint8), "filter bytes at 2^%d bits" % log2_bits)
+        bm = torch.full(((reads.size + 31) // 32,), -1, dtype=torch.int32, device="cuda")
+        hc = torch.full((n_reads,), -1, dtype=torch.int32, device="cuda")
+        f.query_records(_dev(reads), _dev(offs.view(np.int64)), bm, hc)
+        torch.cuda.synchronize()
+        wbm, wc, _ = o.query_records(reads, offs, threads=True)
+        _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "bitmap words at 2^%d bits" % log2_bits)
+        _first_diff(hc.cpu().numpy().view(np.uint32), wc, "hit counts at 2^%d bits" % log2_bits)
     o.close()
