@@ -372,7 +372,7 @@ def run_cuda(args):
         q_kernel_ms.append((mn, n_q_kmers[b])); pack_ms.append(pk); count_ms.append(ct)
     torch.cuda.synchronize()
 
-    ceilings = measure_ceilings(sbf, num_bits // 8) if rank == 0 else None
+    ceilings = measure_ceilings(sbf, num_bits // 8, sampler.index, sm_max_mhz) if rank == 0 else None
 
     # measured statistics of the last query batch: FPR on the uniform reads (odd read index)
     cnt = d_counts.cpu().numpy().view(np.uint32).astype(np.int64)
@@ -565,24 +565,67 @@ def load_pipes(kernel: str):
     return None, None
 
 
-def measure_ceilings(sbf, filter_bytes):
+class NvmlClock:
+    """SM clock of one GPU sampled through NVML every few milliseconds while a block of code runs."""
+
+    def __init__(self, index: int):
+        self.h = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+        except Exception:
+            self.h = None
+
+    def during(self, fn):
+        """Run fn(); return (its result, median SM clock in MHz sampled meanwhile or None)."""
+        if self.h is None:
+            return fn(), None
+        samples, stop = [], threading.Event()
+
+        def loop():
+            while not stop.is_set():
+                try:
+                    samples.append(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                except Exception:
+                    pass
+                time.sleep(0.004)
+        t = threading.Thread(target=loop, daemon=True)
+        t.start()
+        try:
+            out = fn()
+        finally:
+            stop.set()
+            t.join()
+        tail = samples[len(samples) // 3:]          # the first third may still see the idle clock
+        return out, (statistics.median(tail) if tail else None)
+
+
+def measure_ceilings(sbf, filter_bytes, gpu_index, sm_max_mhz):
     """The box's ceilings, measured in THIS run through the library's sbf_ceiling_* entry points: issue rates of
-    one SM sub-partition by instruction mix (warp instructions per clock, counted in SASS) and random 32-byte-sector
-    access rates over an array as large as the filter."""
-    pipes, clk = {}, []
+    one SM sub-partition by instruction mix (warp instructions per second, counted in SASS, divided by the SM clock
+    NVML reports during that very run) and random 32-byte-sector access rates over an array as large as the filter."""
+    nv = NvmlClock(gpu_index)
+    per_s, per_clk, clocks = {}, {}, {}
     for mode in range(sbf.sbf_ceiling_pipe_modes()):
-        r, c = sbf.sbf_ceiling_pipe_rate(mode, 2048)
-        pipes[sbf.sbf_ceiling_pipe_mode_name(mode)] = r
-        clk.append(c)
+        name = sbf.sbf_ceiling_pipe_mode_name(mode)
+        (g_per_s, _c64), mhz = nv.during(lambda: sbf.sbf_ceiling_pipe_rate(mode, 24000))
+        per_s[name] = g_per_s
+        clocks[name] = mhz
+        per_clk[name] = g_per_s * 1e3 / (mhz if mhz else sm_max_mhz)
     names = ["red_or_b64_x4", "red_or_b64_x1", "ld_nc_256", "cp_async_2x16", "tma_reduce_or_32B"]
     rnd = {}
     for mode, nm in enumerate(names):
         try:
             rnd[nm] = sbf.sbf_ceiling_random_sector(mode, min(filter_bytes, 8 << 30))
-        except Exception as e:  # noqa: BLE001 - a ceiling that cannot be measured is reported as such
+        except Exception:  # noqa: BLE001 - a ceiling that cannot be measured is reported as such
             rnd[nm] = None
     return {"source": "measured in this run (sbf_ceiling_pipe_rate / sbf_ceiling_random_sector, include/sbf.h)",
-            "pipe_warp_inst_per_clk_per_smsp": pipes, "sm_clock_mhz_during_pipe_runs": statistics.median(clk),
+            "pipe_g_warp_inst_per_s_per_smsp": per_s, "sm_clock_mhz_during_pipe_runs": clocks,
+            "sm_clock_source": "NVML nvmlDeviceGetClockInfo(SM) sampled every 4 ms during each run"
+            if nv.h is not None else "NVML unavailable: sm_max_mhz assumed",
+            "pipe_warp_inst_per_clk_per_smsp": per_clk,
             "random_sector_g_per_s": rnd, "random_sector_array_bytes": int(min(filter_bytes, 8 << 30))}
 
 

@@ -230,7 +230,7 @@ def sbf_ceiling_pipe_mode_name(mode: int) -> str: return load_library().sbf_ceil
 
 
 def sbf_ceiling_pipe_rate(mode: int, iters: int = 2048):
-    """(warp instructions per clock per SM sub-partition, SM clock in MHz) of one instruction mix."""
+    """(1e9 warp instructions per second per SM sub-partition, clock64() rate in MHz) of one instruction mix."""
     r, c = ctypes.c_double(0), ctypes.c_double(0)
     _check(load_library().sbf_ceiling_pipe_rate(mode, iters, ctypes.addressof(r), ctypes.addressof(c)))
     return float(r.value), float(c.value)

@@ -116,7 +116,7 @@ struct sbf {
     uint16_t *gmask;
     uint64_t cap_words;       // allocated words in packed / gmask
     uint64_t last_words;      // words written by the last pack
-    uint32_t *d_maxlen;       // longest record of the last batch (written by mark_ends_kernel)
+    uint32_t *d_flag;         // record-mode fallback flag of the last query (cleared by pack_kernel, raised by stream_rec_kernel)
     // L2 persistence window (a7)
     bool l2_window;
     cudaStream_t l2_stream_set;
@@ -170,9 +170,11 @@ void apply_l2_window(sbf *f, cudaStream_t st)
     f->l2_stream_valid = true;
 }
 
-// a1: pack + validity mask (+ record ends) of one batch into the scratch
+// a1: pack + validity mask of one batch into the scratch.  Chunk mode over records (rec_bitmap == nullptr) also marks the
+// record ends; record mode (rec_bitmap = the result bitmap) bounds each record by its length instead, and has the
+// pack kernel zero the bitmap and the fallback flag in passing.
 int run_pack(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, cudaStream_t st,
-             bool want_max_len = false)
+             uint32_t *rec_bitmap = nullptr)
 {
     int rc = ensure_scratch(f, total);
     if (rc) return rc;
@@ -181,14 +183,12 @@ int run_pack(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_
     unsigned blocks = (unsigned)(((nw + 1) / 2 + 255) / 256);
     int aligned = ((reinterpret_cast<uintptr_t>(d_bases) & 15) == 0) ? 1 : 0;
     pack_kernel<<<blocks, 256, 0, st>>>(reinterpret_cast<const uint8_t *>(d_bases), total, f->packed, f->gmask, nw, f->k,
-                                        aligned);
+                                        aligned, rec_bitmap, (total + 31) / 32, rec_bitmap ? f->d_flag : nullptr);
     CK(cudaGetLastError());
     g_launches++;
-    if (d_offsets && n_rec > 0 && (f->k >= 2 || want_max_len) && total > 0) {
-        unsigned b2 = (unsigned)((n_rec + 255) / 256);
-        if (want_max_len) CK(cudaMemsetAsync(f->d_maxlen, 0, sizeof(uint32_t), st));
-        mark_ends_kernel<<<b2, 256, 0, st>>>(d_offsets, n_rec, total, reinterpret_cast<uint32_t *>(f->gmask), f->k,
-                                             want_max_len ? f->d_maxlen : nullptr);
+    if (!rec_bitmap && d_offsets && n_rec > 1 && f->k >= 2 && total > 0) {
+        unsigned b2 = (unsigned)((n_rec + 255) / 256 < 4736 ? (n_rec + 255) / 256 : 4736);
+        mark_ends_kernel<<<b2, 256, 0, st>>>(d_offsets, n_rec, total, reinterpret_cast<uint32_t *>(f->gmask), f->k, nullptr);
         CK(cudaGetLastError());
         g_launches++;
     }
@@ -199,7 +199,7 @@ StreamParams make_params(sbf *f, uint64_t total, uint32_t *bitmap)
 {
     StreamParams p;
     p.packed = f->packed;
-    p.gmask = f->gmask;
+    p.vmask = f->gmask;
     p.n_pos = total;
     p.filter = f->filter;
     p.shard_shift = 32 - f->P;
@@ -207,7 +207,7 @@ StreamParams make_params(sbf *f, uint64_t total, uint32_t *bitmap)
     p.n_bitmap_words = (total + 31) / 32;
     // short chunks for small batches, so that the grid still fills 148 SMs x 6 CTAs a few times over
     p.chunk_blocks = total >= (64ull << 20) ? 8 : total >= (16ull << 20) ? 4 : 2;
-    p.offsets = nullptr; p.n_rec = 0; p.counts = nullptr; p.max_len = nullptr; p.rec_limit = 0;
+    p.offsets = nullptr; p.n_rec = 0; p.counts = nullptr; p.fallback = nullptr; p.rec_limit = 0;
     return p;
 }
 
@@ -256,13 +256,13 @@ int run_insert(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t 
 }
 
 int run_count_records(const uint32_t *d_bitmap, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, uint32_t *d_counts,
-                      cudaStream_t st, const uint32_t *max_len = nullptr, uint32_t rec_limit = 0)
+                      cudaStream_t st, const uint32_t *only_if = nullptr)
 {
     if (n_rec == 0) return SBF_OK;
     if (total / n_rec < 2048) {
         unsigned blocks = (unsigned)((n_rec + 255) / 256);
-        if (max_len != nullptr && blocks > 148 * 8) blocks = 148 * 8; // fallback behind record mode: strides
-        count_records_thread_kernel<<<blocks, 256, 0, st>>>(d_bitmap, d_offsets, n_rec, d_counts, max_len, rec_limit);
+        if (only_if != nullptr && blocks > 148 * 8) blocks = 148 * 8; // fallback behind record mode: strides
+        count_records_thread_kernel<<<blocks, 256, 0, st>>>(d_bitmap, d_offsets, n_rec, d_counts, only_if);
     } else {
         unsigned blocks = (unsigned)(n_rec < 4096 ? n_rec : 4096);
         count_records_block_kernel<<<blocks, 256, 0, st>>>(d_bitmap, d_offsets, n_rec, d_counts);
@@ -273,8 +273,9 @@ int run_count_records(const uint32_t *d_bitmap, const uint64_t *d_offsets, uint6
 }
 
 // Record mode (one thread per record, stream_rec_kernel) is tried for batches of short records: the host knows only
-// the MEAN length, so the longest record is found on the device (mark_ends_kernel) and the record-mode kernel and
-// the chunk-mode kernels both look at it: exactly one of the two does the work, the other exits at once.
+// the MEAN length.  A thread that meets a record above kRecMaxLimit raises a device flag instead of walking it, and the
+// chunk-mode launches queued right behind (record-end marking, chunk kernel, count kernel) then redo the whole batch;
+// while the flag is clear they exit at once.  No host synchronisation either way.
 constexpr uint64_t kRecMeanLimit = 400; // symbols
 constexpr uint32_t kRecMaxLimit = 1024; // symbols
 
@@ -286,25 +287,31 @@ int run_query(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n
     const bool try_rec = f->entry && f->entry->query_rec && d_offsets && n_rec > 0 && total / n_rec <= kRecMeanLimit;
     int rc = mark(f, 0, st);
     if (rc) return rc;
-    rc = run_pack(f, d_bases, d_offsets, n_rec, total, st, try_rec);
+    rc = run_pack(f, d_bases, d_offsets, n_rec, total, st, try_rec ? d_bitmap : nullptr);
     if (rc) return rc;
     rc = mark(f, 1, st);
     if (rc) return rc;
     if (try_rec) {
         StreamParams p = make_params(f, total, d_bitmap);
-        p.offsets = d_offsets; p.n_rec = n_rec; p.counts = d_counts; p.max_len = f->d_maxlen; p.rec_limit = kRecMaxLimit;
-        CK(cudaMemsetAsync(d_bitmap, 0, p.n_bitmap_words * sizeof(uint32_t), st)); // record mode ORs into it
+        p.offsets = d_offsets; p.n_rec = n_rec; p.counts = d_counts; p.fallback = f->d_flag; p.rec_limit = kRecMaxLimit;
         CK(f->entry->query_rec(p, st));
-        CK(f->entry->query(p, st)); // exits at once unless a record is longer than kRecMaxLimit
-        g_launches += 2;
+        g_launches++;
         rc = mark(f, 2, st);
         if (rc) return rc;
-        if (d_counts) {
-            rc = run_count_records(d_bitmap, d_offsets, n_rec, total, d_counts, st, f->d_maxlen, kRecMaxLimit);
-            if (rc) return rc;
-            rc = mark(f, 3, st);
+        // the fallback behind record mode: all three exit at once unless a record was longer than kRecMaxLimit
+        if (f->k >= 2 && n_rec > 1) {
+            unsigned b2 = (unsigned)((n_rec + 255) / 256 < 1184 ? (n_rec + 255) / 256 : 1184);
+            mark_ends_kernel<<<b2, 256, 0, st>>>(d_offsets, n_rec, total, reinterpret_cast<uint32_t *>(f->gmask), f->k, f->d_flag);
+            CK(cudaGetLastError());
+            g_launches++;
         }
-        return rc;
+        CK(f->entry->query(p, st));
+        g_launches++;
+        if (d_counts) {
+            rc = run_count_records(d_bitmap, d_offsets, n_rec, total, d_counts, st, f->d_flag);
+            if (rc) return rc;
+        }
+        return mark(f, 3, st);
     }
     rc = run_main<false>(f, total, d_bitmap, st);
     if (rc) return rc;
@@ -356,14 +363,14 @@ sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits)
     f->k = k; f->m = m; f->s = s; f->H = H; f->P = P; f->device = dev;
     f->num_shards = shards;
     f->host_chunk = kHostChunkDefault;
-    f->entry = find_entry(k, m, s, H);
+    f->entry = P < 32 ? find_entry(k, m, s, H) : nullptr; // the specialised kernels take sigma's shift as a multiply by 2^P
     e = cudaMalloc(&f->filter, shards * 32);
     if (e == cudaSuccess) e = cudaMemset(f->filter, 0, shards * 32);
-    if (e == cudaSuccess) e = cudaMalloc(&f->d_maxlen, 256);
+    if (e == cudaSuccess) e = cudaMalloc(&f->d_flag, 256);
     if (e != cudaSuccess) {
         fail_cuda(e, "sbf_create: filter allocation");
         if (f->filter) cudaFree(f->filter);
-        if (f->d_maxlen) cudaFree(f->d_maxlen);
+        if (f->d_flag) cudaFree(f->d_flag);
         delete f;
         return nullptr;
     }
@@ -391,7 +398,7 @@ void sbf_destroy(sbf_t *f)
     if (f->packed) cudaFree(f->packed);
     if (f->gmask) cudaFree(f->gmask);
     if (f->filter) cudaFree(f->filter);
-    if (f->d_maxlen) cudaFree(f->d_maxlen);
+    if (f->d_flag) cudaFree(f->d_flag);
     cudaGetLastError();
     delete f;
 }

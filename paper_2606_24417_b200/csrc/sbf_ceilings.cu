@@ -3,10 +3,12 @@
 // on the same box and clocks as the kernels it times, and writes the results into its JSON line.
 //
 //   sbf_ceiling_pipe_rate      issue rate of one SM sub-partition (SMSP) for a fixed instruction mix, in WARP
-//                              INSTRUCTIONS PER CLOCK, counted in SASS: every loop body below is N x one inline-PTX
+//                              INSTRUCTIONS PER SECOND, counted in SASS: every loop body below is N x one inline-PTX
 //                              instruction that ptxas maps 1:1 to the SASS opcode named in kPipeModeName
-//                              (tests/test_ceilings_sass.py disassembles the object and counts them), and the clock
-//                              is the SM's own cycle counter, so the figure does not depend on the clock frequency.
+//                              (tests/test_ceilings_sass.py disassembles the object and counts them), timed with CUDA
+//                              events.  The caller divides by the SM clock it samples during the run (bench.py: NVML);
+//                              the in-kernel clock64() delta is returned as well, but on this driver that counter does
+//                              not tick at the SM clock (it gave 1.58 warp instructions per "cycle" per SMSP).
 //   sbf_ceiling_random_sector  random 32-byte-sector accesses per second over an array of a given size, with exactly
 //                              the access the fused kernels make (4 x RED.OR.B64 per sector; 2 x 16-byte cp.async; ...)
 #include "../../include/sbf.h"
@@ -87,7 +89,8 @@ constexpr int kRandTPB = 128;
 template <int MODE>
 __global__ void __launch_bounds__(kRandTPB) random_sector_kernel(uint64_t *arr, uint64_t sector_mask, uint32_t per_thread, uint64_t *sink)
 {
-    __shared__ __align__(16) uint64_t stage[2][kRandTPB][4];
+    constexpr int kSlots = 8; // staged sectors in flight per thread (the query kernels keep up to kLA + 1 = 8)
+    __shared__ __align__(16) uint64_t stage[MODE == 3 ? kSlots : 2][kRandTPB][4];
     const uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     uint64_t acc = 0;
     for (uint32_t i = 0; i < per_thread; ++i) {
@@ -104,12 +107,12 @@ __global__ void __launch_bounds__(kRandTPB) random_sector_kernel(uint64_t *arr, 
             asm volatile("ld.global.nc.v4.u64 {%0,%1,%2,%3}, [%4];" : "=l"(w0), "=l"(w1), "=l"(w2), "=l"(w3) : "l"(p));
             acc += w0 ^ w1 ^ w2 ^ w3;
         } else if (MODE == 3) {
-            const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(&stage[i & 1][threadIdx.x][0]);
+            const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(&stage[i % kSlots][threadIdx.x][0]);
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s0), "l"(p) : "memory");
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s0 + 16), "l"(p + 2) : "memory");
             asm volatile("cp.async.commit_group;" ::: "memory");
-            asm volatile("cp.async.wait_group 1;" ::: "memory");   // the previous iteration's sector has landed
-            acc += stage[(i & 1) ^ 1][threadIdx.x][0] ^ stage[(i & 1) ^ 1][threadIdx.x][3];
+            asm volatile("cp.async.wait_group 7;" ::: "memory");   // the sector staged kSlots - 1 iterations ago has landed
+            acc += stage[(i + 1) % kSlots][threadIdx.x][0] ^ stage[(i + 1) % kSlots][threadIdx.x][3];
         } else {
             asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory"); // the slot used two iterations ago is free
             uint64_t *s = &stage[i & 1][threadIdx.x][0];
@@ -146,9 +149,9 @@ extern "C" {
 int sbf_ceiling_pipe_modes(void) { return kPipeModes; }
 const char *sbf_ceiling_pipe_mode_name(int mode) { return (mode >= 0 && mode < kPipeModes) ? kPipeModeName[mode] : ""; }
 
-int sbf_ceiling_pipe_rate(int mode, int iters, double *warp_inst_per_clk_per_smsp, double *sm_clock_mhz)
+int sbf_ceiling_pipe_rate(int mode, int iters, double *g_warp_inst_per_s_per_smsp, double *clock64_mhz)
 {
-    if (mode < 0 || mode >= kPipeModes || iters < 1 || !warp_inst_per_clk_per_smsp) return SBF_ERR_INVALID_ARG;
+    if (mode < 0 || mode >= kPipeModes || iters < 1 || !g_warp_inst_per_s_per_smsp) return SBF_ERR_INVALID_ARG;
     int dev = 0, sms = 0;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
         return SBF_ERR_CUDA;
@@ -193,8 +196,8 @@ int sbf_ceiling_pipe_rate(int mode, int iters, double *warp_inst_per_clk_per_sms
     // all CTAs are resident at once: every SMSP holds kPipeCTAsPerSM * 8 / 4 warps for the whole run
     const double warps_per_smsp = kPipeCTAsPerSM * (kPipeTPB / 32) / 4.0;
     const double inst_per_warp = (double)iters * kPipeUnroll * kPipeChains;
-    *warp_inst_per_clk_per_smsp = warps_per_smsp * inst_per_warp / best_cycles;
-    if (sm_clock_mhz) *sm_clock_mhz = best_cycles / (best_ms * 1e-3) / 1e6; // loop cycles / kernel time: a lower bound of the clock
+    *g_warp_inst_per_s_per_smsp = warps_per_smsp * inst_per_warp / (best_ms * 1e-3) / 1e9;
+    if (clock64_mhz) *clock64_mhz = best_cycles / (best_ms * 1e-3) / 1e6; // rate of the in-kernel cycle counter
     return SBF_OK;
 }
 

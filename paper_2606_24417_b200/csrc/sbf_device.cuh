@@ -5,8 +5,10 @@
 //
 // Kernels
 //   pack_kernel        a1  ASCII -> 2-bit words (16 bases / uint32, first base in the top bits)
-//                          + "k-mer cannot start here" mask G (1 bit / base)
-//   mark_ends_kernel   a1  ORs the record-end bits into G
+//                          + V, one bit per base: "no valid k-mer starts here" (a non-ACGT symbol among the
+//                          next k, or fewer than k symbols left)
+//   mark_ends_kernel   a1  chunk mode over records: ORs into V the k-1 start positions before every record
+//                          end (a k-mer never spans two records)
 //   stream_kernel      a2-a6  the fused, thread-serial streaming insert / query kernel
 //   naive_kernel       a2-a6  runtime-parameter one-k-mer-per-thread form of Alg. 1/2 (any legal k,m,s,H)
 //   count kernels      a6  per-record / total popcount of the result bitmap
@@ -22,13 +24,19 @@
 #define SBF_MINB_R 4 // record-mode query: 4 x 128 threads -> 128 registers
 #endif
 #ifndef SBF_Q_LA
-#define SBF_Q_LA 3   // query: the minimizer runs this many positions ahead of the bit tests
-#endif
-#ifndef SBF_Q_PF
-#define SBF_Q_PF 3   // query (chunk mode): 0 load at first use, 1 prefetch.global.L2 ahead, 3 cp.async staging in shared memory
+#define SBF_Q_LA 7   // query: the minimizer runs this many positions ahead of the bit tests (1, 3, 7: 7 measured best)
 #endif
 #ifndef SBF_IDP_EXTRACT
 #define SBF_IDP_EXTRACT 1 // bit-slice extraction by IDP.4A where the slice is byte aligned (H = 1, 2, 4, 8)
+#endif
+#ifndef SBF_FMA_ONEHOT
+#define SBF_FMA_ONEHOT 0  // one-hot masks with one alu shift + three fma-pipe multiplies instead of two alu shifts (measured slower: more instructions)
+#endif
+#ifndef SBF_FMA_SIGMA
+#define SBF_FMA_SIGMA 0   // sigma's final shift as a multiply-high by 2^P (fma pipe; measured: no gain)
+#endif
+#ifndef SBF_PRED_RELOAD
+#define SBF_PRED_RELOAD 1 // query: reload the shard registers with two predicated LDS.128 instead of a divergent branch
 #endif
 #ifndef SBF_MINB_I
 #define SBF_MINB_I 5 // insert: CTAs per SM the register budget is cut for (5 x 128 threads -> 96 registers)
@@ -53,7 +61,7 @@ constexpr int kPadWords = 16;   // zero / all-invalid words appended to the pack
 
 struct StreamParams {
     const uint32_t *packed; // 2-bit words, ceil(n_pos/16) + kPadWords
-    const uint16_t *gmask;  // one uint16 per packed word: bit j = G[16*word + j]
+    const uint16_t *vmask;  // one uint16 per packed word: bit j = V[16*word + j], "no valid k-mer starts at that symbol"
     uint64_t n_pos;         // symbols in the batch (= k-mer start positions walked)
     uint64_t *filter;       // 4 * numShards sector words
     int shard_shift;        // 32 - P
@@ -63,8 +71,8 @@ struct StreamParams {
     const uint64_t *offsets; // n_rec + 1
     uint64_t n_rec;
     uint32_t *counts;        // nullable: per-record hit counts
-    const uint32_t *max_len; // device word written by mark_ends_kernel: longest record of the batch
-    uint32_t rec_limit;      // record mode runs iff *max_len <= rec_limit (the chunk kernels run otherwise)
+    uint32_t *fallback;      // device flag: record mode met a record above rec_limit -> the chunk kernels redo the batch
+    uint32_t rec_limit;      // longest record one thread of stream_rec_kernel walks
     int chunk_blocks;        // chunk mode: 16-position blocks walked by one thread (2, 4 or 8: small batches use short chunks)
 };
 
@@ -133,11 +141,11 @@ __device__ __forceinline__ void red_or_64(uint64_t *p, uint64_t v)
 }
 
 // =============================================================================================
-// a1: pack.  Thread i produces packed words 2i, 2i+1 and their mask words from symbols [32i, 32i+32).
+// a1: pack.  Thread i produces packed words 2i, 2i+1 and the 32 V bits of symbols [32i, 32i+32).
 //   code: A=0 C=1 G=2 T=3 (either case, A9); anything else is invalid (code bits arbitrary).
-//   B[j] = symbol j invalid or j >= len.   G[j] = B[j] | B[j+1] (k >= 2), = B[j] (k == 1).
-//   A k-mer starting at p is valid iff G[p .. p+max(k-1,1)-1] are all 0 once mark_ends_kernel
-//   has added F[j] = "a record ends after symbol j" (no k-mer spans records).
+//   B[j] = symbol j is not ACGT, or j >= len.   V[j] = B[j] | B[j+1] | ... | B[j+k-1]:
+//   no valid k-mer starts at symbol j.  Record ends are not known here: record mode bounds each
+//   record by its own length, chunk mode over records adds them with mark_ends_kernel.
 // =============================================================================================
 __device__ __forceinline__ uint32_t pack4(uint32_t v, uint32_t &inv4)
 {
@@ -157,13 +165,9 @@ __device__ __forceinline__ uint32_t pack4(uint32_t v, uint32_t &inv4)
 }
 
 #ifdef SBF_DEFINE_AUX_KERNELS // non-template kernels: defined in one translation unit (sbf_api.cu)
-__global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ seq, uint64_t len, uint32_t *__restrict__ packed,
-                                                   uint16_t *__restrict__ gmask, uint64_t n_words_total, int k, int aligned16)
+// 32 symbols starting at b0 as eight little-endian 4-byte groups ('N' past the end)
+__device__ __forceinline__ void load32(const uint8_t *__restrict__ seq, uint64_t b0, uint64_t len, int aligned16, uint32_t (&v)[8])
 {
-    // thread i: symbols [32i, 32i+32) -> packed words 2i, 2i+1 (one 8-byte store) and their two mask words (one 4-byte store)
-    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const uint64_t b0 = i * 32;
-    uint32_t v[8];
     if (aligned16 && b0 + 32 <= len) {
         const uint4 q0 = __ldg(reinterpret_cast<const uint4 *>(seq + b0));
         const uint4 q1 = __ldg(reinterpret_cast<const uint4 *>(seq + b0 + 16));
@@ -182,6 +186,22 @@ __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ s
             v[w] = acc;
         }
     }
+}
+
+// bitmap_zero (nullable): the result bitmap of a record-mode query, whose word i covers exactly this thread's 32
+// symbols — zeroed here, in passing, because record mode ORs into the words two records share.
+// flag_zero (nullable): the record-mode fallback flag, cleared by the first thread.
+__global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ seq, uint64_t len, uint32_t *__restrict__ packed,
+                                                   uint16_t *__restrict__ vmask, uint64_t n_words_total, int k, int aligned16,
+                                                   uint32_t *__restrict__ bitmap_zero, uint64_t n_bitmap_words,
+                                                   uint32_t *__restrict__ flag_zero)
+{
+    // thread i: symbols [32i, 32i+32) -> packed words 2i, 2i+1 (one 8-byte store) and their two mask words (one 4-byte store)
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint64_t b0 = i * 32;
+    if (i == 0 && flag_zero != nullptr) *flag_zero = 0;
+    uint32_t v[8];
+    load32(seq, b0, len, aligned16, v);
     uint32_t word[2] = {0, 0}, inv = 0;
 #pragma unroll
     for (int w = 0; w < 8; ++w) {
@@ -190,44 +210,52 @@ __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ s
         word[w >> 2] |= c8 << (24 - 8 * (w & 3));
         inv |= i4 << (4 * w);
     }
-    // B of the next symbol: first flag of the next lane, or a direct byte load at the warp edge
-    uint32_t nxt = __shfl_down_sync(0xFFFFFFFFu, inv & 1u, 1);
+    // B of the next 32 symbols: the next lane's word, or (last lane of the warp) classified here
+    uint32_t nxt = __shfl_down_sync(0xFFFFFFFFu, inv, 1);
     if ((threadIdx.x & 31) == 31) {
-        const uint64_t p = b0 + 32;
-        uint32_t c = (p < len) ? (uint32_t)seq[p] : (uint32_t)'N';
-        c &= 0xDFu;
-        nxt = !(c == 'A' || c == 'C' || c == 'G' || c == 'T');
-    }
-    const uint32_t g = (k >= 2) ? (inv | (inv >> 1) | (nxt << 31)) : inv;
-    if (2 * i + 1 < n_words_total) {
-        *reinterpret_cast<uint2 *>(packed + 2 * i) = make_uint2(word[0], word[1]);
-        *reinterpret_cast<uint32_t *>(gmask + 2 * i) = g;
-    } else if (2 * i < n_words_total) {
-        packed[2 * i] = word[0];
-        gmask[2 * i] = (uint16_t)g;
-    }
-}
-
-// F bits: a record boundary after symbol offsets[r]-1, r = 1..n_rec  (k >= 2 only); also the longest
-// record of the batch -> *max_len (nullable), which selects record mode or chunk mode on the device.
-__global__ void __launch_bounds__(256) mark_ends_kernel(const uint64_t *__restrict__ offsets, uint64_t n_rec, uint64_t total,
-                                                        uint32_t *gmask32, int k, uint32_t *max_len)
-{
-    const uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x + 1;
-    uint32_t len = 0;
-    if (r <= n_rec) {
-        const uint64_t e = offsets[r], a = offsets[r - 1];
-        const uint64_t l64 = e >= a ? e - a : 0;
-        len = l64 > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)l64;
-        if (k >= 2 && e != 0 && e <= total) {
-            const uint64_t j = e - 1;
-            atomicOr(&gmask32[j >> 5], 1u << (j & 31));
+        load32(seq, b0 + 32, len, aligned16, v);
+        nxt = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) {
+            uint32_t i4;
+            (void)pack4(v[w], i4);
+            nxt |= i4 << (4 * w);
         }
     }
-    if (max_len != nullptr) {
-        // one atomic per warp, and only while it can still raise the maximum (monotone, so the stale read is safe)
-        len = __reduce_max_sync(0xFFFFFFFFu, len);
-        if ((threadIdx.x & 31) == 0 && len > *reinterpret_cast<volatile uint32_t *>(max_len)) atomicMax(max_len, len);
+    // V = OR of k consecutive B bits, by doubling: after the loop bit j of y covers B[j .. j+c-1], c the largest power
+    // of two <= k; one more step with the remainder closes the window (k - c <= c)
+    uint64_t y = (uint64_t)inv | ((uint64_t)nxt << 32);
+    int c = 1;
+    while (2 * c <= k) {
+        y |= y >> c;
+        c *= 2;
+    }
+    if (c < k) y |= y >> (k - c);
+    const uint32_t g = (uint32_t)y;
+    if (2 * i + 1 < n_words_total) {
+        *reinterpret_cast<uint2 *>(packed + 2 * i) = make_uint2(word[0], word[1]);
+        *reinterpret_cast<uint32_t *>(vmask + 2 * i) = g;
+    } else if (2 * i < n_words_total) {
+        packed[2 * i] = word[0];
+        vmask[2 * i] = (uint16_t)g;
+    }
+    if (bitmap_zero != nullptr && i < n_bitmap_words) bitmap_zero[i] = 0;
+}
+
+// Chunk mode over a record batch: the k-1 start positions before a record end e = offsets[r] (r = 1..n_rec) have no
+// k-mer (it would span two records): OR the bit range [e-(k-1), e) into V.  only_if (nullable): the record-mode
+// fallback flag — the launch does nothing unless it is set.
+__global__ void __launch_bounds__(256) mark_ends_kernel(const uint64_t *__restrict__ offsets, uint64_t n_rec, uint64_t total,
+                                                        uint32_t *vmask32, int k, const uint32_t *only_if)
+{
+    if (only_if != nullptr && *only_if == 0) return;
+    for (uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x + 1; r <= n_rec; r += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t e = offsets[r];
+        if (k < 2 || e == 0 || e > total) continue;
+        const uint64_t lo = e >= (uint64_t)(k - 1) ? e - (uint64_t)(k - 1) : 0;
+        const uint64_t mask = (((uint64_t)1 << (e - lo)) - 1) << (lo & 31); // at most 31 bits, spanning at most two words
+        atomicOr(&vmask32[lo >> 5], (uint32_t)mask);
+        if (mask >> 32) atomicOr(&vmask32[(lo >> 5) + 1], (uint32_t)(mask >> 32));
     }
 }
 
@@ -301,6 +329,73 @@ struct SlidingMin {
     }
 };
 
+// Sliding OR of the last WO masks (WO = k-s+1: the k-mer's mask K is the OR of its s-mers' one-hot masks), streaming like
+// SlidingMin: c3 = OR of the last 3, c9 = OR of the last 9, the window covered by two or three overlapping blocks —
+// overlap is free for OR, and a three-input OR (or OR-then-AND-NOT) is one LOP3.  push_test() returns the bits of K
+// that are NOT set in the shard (all zero = every s-mer of the k-mer hits, the Findere rule).
+template <int WO, int NW>
+struct SlidingOr {
+    static_assert(WO >= 1 && WO <= 17, "stream kernels support k-s <= 16");
+    uint64_t m[16][NW], c3[16][NW], c9[16][NW];
+    __device__ __forceinline__ void clear()
+    {
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+#pragma unroll
+            for (int q = 0; q < NW; ++q) { m[i][q] = 0; c3[i][q] = 0; c9[i][q] = 0; }
+    }
+    template <int E>
+    __device__ __forceinline__ uint64_t window(const uint64_t (&Mn)[NW], int q)
+    {
+        constexpr int e = E & 15;
+        m[e][q] = Mn[q];
+        if constexpr (WO == 1) return Mn[q];
+        if constexpr (WO == 2) return Mn[q] | m[(E - 1) & 15][q];
+        const uint64_t a3 = Mn[q] | m[(E - 1) & 15][q] | m[(E - 2) & 15][q];
+        c3[e][q] = a3;
+        if constexpr (WO == 3) return a3;
+        if constexpr (WO >= 4 && WO <= 6) return a3 | c3[(E - (WO - 3)) & 15][q];
+        if constexpr (WO >= 7 && WO <= 9) return a3 | c3[(E - 3) & 15][q] | c3[(E - (WO - 3)) & 15][q];
+        if constexpr (WO >= 10) {
+            const uint64_t a9 = a3 | c3[(E - 3) & 15][q] | c3[(E - 6) & 15][q];
+            c9[e][q] = a9;
+            return a9 | c9[(E - (WO - 9)) & 15][q];
+        }
+        return a3;
+    }
+    template <int E>
+    __device__ __forceinline__ void push(const uint64_t (&Mn)[NW])
+    {
+#pragma unroll
+        for (int q = 0; q < NW; ++q) (void)window<E>(Mn, q);
+    }
+    template <int E>
+    __device__ __forceinline__ uint64_t push_test(const uint64_t (&Mn)[NW], const uint64_t (&shard)[4])
+    {
+        uint64_t miss = 0;
+#pragma unroll
+        for (int q = 0; q < NW; ++q) miss |= window<E>(Mn, q) & ~shard[q];
+        return miss;
+    }
+};
+
+// 1 << b for b in [0, 64) as two 32-bit halves.  SBF_FMA_ONEHOT: one shift on the alu pipe (1 << (b & 31)), the
+// half it belongs to picked by multiplications (b >> 5 as a multiply-high, then x * {0,1} and x - y as IMADs), which
+// issue on the fma pipe — the stream kernels are bound by the alu pipe, the fma pipe is two thirds idle.
+__device__ __forceinline__ uint64_t onehot64(uint32_t b)
+{
+#if SBF_FMA_ONEHOT
+    const uint32_t m32 = 1u << (b & 31u);
+    const uint32_t b5 = __umulhi(b, 0x08000000u); // b >> 5
+    uint32_t hi, lo;
+    asm("mul.lo.u32 %0, %1, %2;" : "=r"(hi) : "r"(m32), "r"(b5));
+    asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(lo) : "r"(hi), "r"(0xFFFFFFFFu), "r"(m32)); // m32 - hi
+    return ((uint64_t)hi << 32) | lo;
+#else
+    return 1ull << b;
+#endif
+}
+
 // One-hot sector masks of one s-mer hash: hash index i -> word i mod 4, bit B(h,i) (A5)
 template <int OFF>
 __device__ __forceinline__ uint64_t onehot_at(uint64_t h)
@@ -310,11 +405,10 @@ __device__ __forceinline__ uint64_t onehot_at(uint64_t h)
         // byte-aligned slice: mask all four bytes of the half at once (shared by the other slices of that half), then
         // pick the byte with a byte dot product (IDP.4A runs off the alu pipe that bounds the query kernels)
         const uint32_t half = OFF < 32 ? (uint32_t)h : (uint32_t)(h >> 32);
-        const uint32_t b = __dp4a(half & 0x3F3F3F3Fu, 1u << (OFF % 32), 0u);
-        return 1ull << b;
+        return onehot64(__dp4a(half & 0x3F3F3F3Fu, 1u << (OFF % 32), 0u));
     }
 #endif
-    return 1ull << ((h >> OFF) & 63);
+    return onehot64((uint32_t)(h >> OFF) & 63u);
 }
 
 template <int H, int NW>
@@ -332,15 +426,24 @@ __device__ __forceinline__ void expand_masks(uint64_t h, uint64_t (&m)[NW])
 
 __host__ __device__ constexpr int ring_size(int z) { return z <= 1 ? 1 : z <= 2 ? 2 : z <= 4 ? 4 : z <= 8 ? 8 : 16; }
 
-// A2 with the shift clamped in hardware (shard_shift = 32 when there is one shard)
+// A2.  shard_shift = 32 - P (32 when there is one shard).  The final shift t >> (32 - P) is a multiply-high by 2^P
+// on the fma pipe (specialised kernels serve P <= 31; 2^32 shards run the runtime-parameter kernel).
 __device__ __forceinline__ uint32_t sigma32(uint32_t key, int shard_shift)
 {
     uint32_t t = (uint32_t)(((uint64_t)key * kGold64) >> 32);
+#if SBF_FMA_SIGMA
+    return __umulhi(t, 1u << ((32 - shard_shift) & 31));
+#else
     return __funnelshift_rc(t, 0u, (uint32_t)shard_shift);
+#endif
 }
 
-// query staging through shared memory (SBF_Q_PF == 3): the 32 bytes of a shard travel global -> shared with two
-// 16-byte cp.async (LDGSTS, no register in between) LA positions before the run's first test reads them back.
+// query staging through shared memory: the 32 bytes of a shard travel global -> shared with two 16-byte cp.async
+// (LDGSTS, no register in between) kLA positions before the run's first test reads them back.
+constexpr int kLA = SBF_Q_LA; // the minimizer runs this many positions ahead of the bit tests
+constexpr int kNS = kLA + 1;  // staging slots per thread: k-mer q uses slot q mod kNS
+static_assert(kLA >= 1 && 16 % kNS == 0, "staging needs a look-ahead of 1, 3, 7 or 15");
+
 __device__ __forceinline__ void cp_async_shard(uint4 *smem_lo, uint4 *smem_hi, const uint64_t *g)
 {
     uint32_t a = (uint32_t)__cvta_generic_to_shared(smem_lo), b = (uint32_t)__cvta_generic_to_shared(smem_hi);
@@ -351,21 +454,100 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-__device__ __forceinline__ void prefetch_shard(const uint64_t *p)
-{
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-}
+// The query pipeline of one thread (shared by chunk mode and record mode): minimizer + shard of k-mer q+kLA, staging
+// of a new run's sector, the newest s-mer's masks, the k-mer test of k-mer q.  Validity plays no part here: a
+// position without a valid k-mer computes on whatever symbols are there (its shard index is still in range) and its
+// result bit is cleared from V afterwards, 16 positions at a time.
+template <int K, int M, int S, int H>
+struct QueryLane {
+    static constexpr int WN = K - M + 1, Z = K - S, NW = H < 4 ? H : 4;
+    SlidingMin<WN> smin;
+    SlidingOr<Z + 1, NW> sor;
+    uint32_t sh32[8]; // the current shard's four sector words as 32-bit halves (little-endian)
+    uint32_t laPrev;
+    bool sb[kNS]; // sb[q mod kNS]: a run starts at k-mer q (its sector is in staging slot q mod kNS)
+
+    // keys of the first WN-1 m-mers, masks of the first Z s-mers, shards of the first kLA k-mers
+    __device__ __forceinline__ void prologue(const uint32_t (&W)[4], const StreamParams &prm, uint4 *stage)
+    {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) { smin.g[i] = 0; smin.c3[i] = 0; smin.c9[i] = 0; }
+        sor.clear();
+#pragma unroll
+        for (int q = 0; q < 8; ++q) sh32[q] = 0;
+#pragma unroll
+        for (int i = 0; i < kNS; ++i) sb[i] = false;
+        laPrev = 0;
+        static_for<0, WN - 1>([&](auto ec) {
+            constexpr int E = decltype(ec)::value;
+            (void)smin.template push<E>(g_key(lmer<E, M>(W), M));
+        });
+        static_for<0, Z>([&](auto ic) {
+            constexpr int I = decltype(ic)::value;
+            uint64_t Mi[NW];
+            expand_masks<H, NW>(f_hash_c<S>(lmer<I, S>(W)), Mi);
+            sor.template push<I>(Mi);
+        });
+        static_for<0, kLA>([&](auto qc) { this->template look<decltype(qc)::value, decltype(qc)::value == 0>(W, prm, stage); });
+    }
+    // k-mer Q (relative to the window): its shard; a change of shard starts a run and stages that sector
+    template <int Q, bool FIRST>
+    __device__ __forceinline__ void look(const uint32_t (&W)[4], const StreamParams &prm, uint4 *stage)
+    {
+        const uint32_t shNew = sigma32(smin.template push<Q + WN - 1>(g_key(lmer<Q + WN - 1, M>(W), M)), prm.shard_shift);
+        const bool start = FIRST || shNew != laPrev;
+        if (start)
+            cp_async_shard(&stage[((Q % kNS) * 2) * kStreamTPB + threadIdx.x], &stage[((Q % kNS) * 2 + 1) * kStreamTPB + threadIdx.x],
+                           prm.filter + (uint64_t)shNew * 4);
+        cp_async_commit();
+        sb[Q % kNS] = start;
+        laPrev = shNew;
+    }
+    // k-mer J of the current 16-position block: returns true iff all its H(k-s+1) bits are set in its shard
+    template <int J>
+    __device__ __forceinline__ bool step(const uint32_t (&W)[4], const StreamParams &prm, uint4 *stage)
+    {
+        this->template look<J + kLA, false>(W, prm, stage);
+        uint64_t Mn[NW];
+        expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
+        // a6: if a run starts here, its sector was staged kLA positions ago: take it into the shard registers
+#if SBF_PRED_RELOAD
+        // almost every warp has SOME lane starting a run at any given position, so a branch would be taken (and its
+        // BSSY/BSYNC paid) nearly always: wait unconditionally, load under a predicate
+        cp_async_wait<kLA>();
+        {
+            const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(&stage[((J % kNS) * 2) * kStreamTPB + threadIdx.x]);
+            const uint32_t a1 = (uint32_t)__cvta_generic_to_shared(&stage[((J % kNS) * 2 + 1) * kStreamTPB + threadIdx.x]);
+            asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %8, 0;\n\t"
+                         "@p ld.shared.v4.u32 {%0,%1,%2,%3}, [%9];\n\t@p ld.shared.v4.u32 {%4,%5,%6,%7}, [%10];\n\t}"
+                         : "+r"(sh32[0]), "+r"(sh32[1]), "+r"(sh32[2]), "+r"(sh32[3]), "+r"(sh32[4]), "+r"(sh32[5]), "+r"(sh32[6]),
+                           "+r"(sh32[7])
+                         : "r"((uint32_t)sb[J % kNS]), "r"(a0), "r"(a1)
+                         : "memory");
+        }
+#else
+        if (sb[J % kNS]) {
+            cp_async_wait<kLA>();
+            const uint4 lo = stage[((J % kNS) * 2) * kStreamTPB + threadIdx.x];
+            const uint4 hi = stage[((J % kNS) * 2 + 1) * kStreamTPB + threadIdx.x];
+            sh32[0] = lo.x; sh32[1] = lo.y; sh32[2] = lo.z; sh32[3] = lo.w;
+            sh32[4] = hi.x; sh32[5] = hi.y; sh32[6] = hi.z; sh32[7] = hi.w;
+        }
+#endif
+        const uint64_t shard[4] = {((uint64_t)sh32[1] << 32) | sh32[0], ((uint64_t)sh32[3] << 32) | sh32[2],
+                                   ((uint64_t)sh32[5] << 32) | sh32[4], ((uint64_t)sh32[7] << 32) | sh32[6]};
+        return sor.template push_test<J + Z>(Mn, shard) == 0;
+    }
+};
 
 // =============================================================================================
-// a2-a6 fused.  One thread walks kChunk consecutive k-mer start positions p0 .. p0+kChunk-1 of the
+// a2-a6 fused, CHUNK MODE.  One thread walks 16 * chunk_blocks consecutive k-mer start positions of the
 // batch, carrying in registers: the 64-symbol window, the sliding-minimum rings (a2), the one-hot
 // masks of the last k-s s-mers, and
 //   insert: the OR of the current super-k-mer's masks (a5), flushed with one RED.OR.B64 per sector
 //           word when the shard (A14) or validity changes;
-//   query : the current shard's 256 bits (a6), reloaded when the shard changes; the k-mer's mask
-//           K = OR of its k-s+1 s-mer masks is tested with K & ~shard == 0 (Findere rule).
-//           The minimizer runs LA positions ahead of the tests so that the shard of an upcoming
-//           run can be prefetched long before its first test.
+//   query : the current shard's 256 bits (a6) and the sliding OR of the k-mer mask K, tested with
+//           K & ~shard == 0 (Findere rule); see QueryLane.
 // Each m-mer key and each s-mer hash is computed once per position (not once per k-mer as in
 // Alg. 1/2); the result bits are the same because OR/AND do not care about order or repetition.
 // =============================================================================================
@@ -376,15 +558,12 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
     constexpr int Z = K - S;
     constexpr int NW = H < 4 ? H : 4;
     constexpr int RZ = ring_size(Z);
-    constexpr int L = K > 1 ? K - 1 : 1;
-    constexpr int LA = INSERT ? 0 : SBF_Q_LA;
-    constexpr uint32_t maskL = (L >= 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
     static_assert(K >= 1 && K <= 32 && M >= 1 && M <= K && S >= 1 && S <= K, "bad k/m/s");
     static_assert(Z <= 16, "stream kernel supports k-s <= 16");
-    static_assert(LA >= 0 && LA <= 16 && (LA == 0 || SBF_Q_PF == 3 || 16 % LA == 0), "lookahead must divide 16");
+    __shared__ uint4 stage[INSERT ? 1 : kNS * 2 * kStreamTPB];
 
     if constexpr (!INSERT) {
-        if (prm.max_len != nullptr && __ldg(prm.max_len) <= prm.rec_limit) return; // stream_rec_kernel did this batch
+        if (prm.fallback != nullptr && *prm.fallback == 0) return; // stream_rec_kernel did this batch
     }
     // one chunk per thread; the (normally idle) fallback launch behind record mode uses a small grid and strides
     for (uint64_t chunk = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;; chunk += (uint64_t)gridDim.x * blockDim.x) {
@@ -392,111 +571,43 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
     if (p0 >= prm.n_pos) return;
 
     const uint32_t *__restrict__ pw = prm.packed + (p0 >> 4);
-    const uint16_t *__restrict__ gw = prm.gmask + (p0 >> 4);
+    const uint16_t *__restrict__ vw = prm.vmask + (p0 >> 4);
     uint32_t W[kWin] = {__ldg(pw), __ldg(pw + 1), __ldg(pw + 2), __ldg(pw + 3)};
-    uint32_t glo = (uint32_t)__ldg(gw) | ((uint32_t)__ldg(gw + 1) << 16);
-    uint32_t ghi = (uint32_t)__ldg(gw + 2) | ((uint32_t)__ldg(gw + 3) << 16);
 
-    SlidingMin<WN> smin;
+    if constexpr (INSERT) {
+        SlidingMin<WN> smin;
 #pragma unroll
-    for (int i = 0; i < 16; ++i) { smin.g[i] = 0; smin.c3[i] = 0; smin.c9[i] = 0; }
-    uint64_t Mh[RZ][NW];
+        for (int i = 0; i < 16; ++i) { smin.g[i] = 0; smin.c3[i] = 0; smin.c9[i] = 0; }
+        uint64_t Mh[RZ][NW]; // masks of the last k-s s-mers: what a new run shares with the k-mers before it
 #pragma unroll
-    for (int i = 0; i < RZ; ++i)
+        for (int i = 0; i < RZ; ++i)
 #pragma unroll
-        for (int q = 0; q < NW; ++q) Mh[i][q] = 0;
-
-    // prologue: keys of the first WN-1 m-mers, masks of the first Z s-mers
-    static_for<0, WN - 1>([&](auto ec) {
-        constexpr int E = decltype(ec)::value;
-        (void)smin.template push<E>(g_key(lmer<E, M>(W), M));
-    });
-    static_for<0, Z>([&](auto ic) {
-        constexpr int I = decltype(ic)::value;
-        expand_masks<H, NW>(f_hash_c<S>(lmer<I, S>(W)), Mh[I % RZ]);
-    });
-    uint64_t PB[NW], PC[NW]; // query, Z == 3: ORs of adjacent mask pairs (see the test below)
+            for (int q = 0; q < NW; ++q) Mh[i][q] = 0;
+        static_for<0, WN - 1>([&](auto ec) {
+            constexpr int E = decltype(ec)::value;
+            (void)smin.template push<E>(g_key(lmer<E, M>(W), M));
+        });
+        static_for<0, Z>([&](auto ic) {
+            constexpr int I = decltype(ic)::value;
+            expand_masks<H, NW>(f_hash_c<S>(lmer<I, S>(W)), Mh[I % RZ]);
+        });
+        uint64_t acc[NW]; // OR of the current run's masks
 #pragma unroll
-    for (int q = 0; q < NW; ++q) {
-        PB[q] = Mh[0][q] | Mh[1 % RZ][q];
-        PC[q] = Mh[1 % RZ][q] | Mh[2 % RZ][q];
-    }
-    // query: shards of the first LA k-mers, prefetched (PF 1/2) or staged in shared memory (PF 3)
-    constexpr bool STAGE = !INSERT && SBF_Q_PF == 3;
-    constexpr int NS = LA + 1; // staging slots per thread: k-mer q uses slot q mod NS
-    static_assert(!STAGE || (LA >= 1 && 16 % NS == 0), "staging needs LA in {1,3,7,15}");
-    __shared__ uint4 stage[STAGE ? NS * 2 * kStreamTPB : 1];
-    uint32_t kq[LA > 0 ? LA : 1];
-    uint32_t laPrev = 0xFFFFFFFFu;
-    bool sb[NS]; // sb[q mod NS]: a run starts at k-mer q (its shard is in staging slot q mod NS)
-#pragma unroll
-    for (int i = 0; i < NS; ++i) sb[i] = false;
-    bool laInv = true;
-    (void)laPrev; (void)sb; (void)laInv; (void)stage;
-    kq[0] = 0;
-    static_for<0, LA>([&](auto ec) {
-        constexpr int Q = decltype(ec)::value;
-        constexpr int E = Q + WN - 1;
-        const uint32_t sh = sigma32(smin.template push<E>(g_key(lmer<E, M>(W), M)), prm.shard_shift);
-        if constexpr (STAGE) {
-            const bool invN = (__funnelshift_r(glo, ghi, Q) & maskL) != 0;
-            const bool start = !invN && (laInv || sh != laPrev);
-            if (start)
-                cp_async_shard(&stage[((Q % NS) * 2) * kStreamTPB + threadIdx.x], &stage[((Q % NS) * 2 + 1) * kStreamTPB + threadIdx.x],
-                               prm.filter + (uint64_t)sh * 4);
-            cp_async_commit();
-            sb[Q % NS] = start;
-            laInv = invN;
-        } else {
-            kq[Q] = sh;
-            if (SBF_Q_PF != 0 && (Q == 0 || sh != laPrev)) prefetch_shard(prm.filter + (uint64_t)sh * 4);
-        }
-        laPrev = sh;
-    });
-
-    uint64_t acc[NW];   // insert: OR of the current run's masks
-    uint64_t shard[4];  // query: the current shard's sector words
-#pragma unroll
-    for (int q = 0; q < NW; ++q) acc[q] = 0;
-#pragma unroll
-    for (int q = 0; q < 4; ++q) shard[q] = 0;
-    uint32_t prevShard = 0;
-    bool prevInval = true; // insert: previous k-mer invalid; query: no shard loaded yet
-    uint32_t res = 0;
-
-    for (int b = 0; b < prm.chunk_blocks; ++b) {
-        const uint32_t wnext = __ldg(pw + b + 4);
-        const uint32_t gnext = __ldg(gw + b + 4);
-        uint32_t res16 = 0;
-        static_for<0, 16>([&](auto jc) {
-            constexpr int J = decltype(jc)::value;
-            // a2/a3: key of the newest m-mer of k-mer p+LA (p = p0+16b+J), its window minimum, its shard
-            const uint32_t shNew =
-                sigma32(smin.template push<J + LA + WN - 1>(g_key(lmer<J + LA + WN - 1, M>(W), M)), prm.shard_shift);
-            uint32_t sh = shNew;
-            (void)sh;
-            if constexpr (STAGE) {
-                const bool invN = (__funnelshift_r(glo, ghi, J + LA) & maskL) != 0;
-                const bool start = !invN && (laInv || shNew != laPrev);
-                if (start)
-                    cp_async_shard(&stage[(((J + LA) % NS) * 2) * kStreamTPB + threadIdx.x],
-                                   &stage[(((J + LA) % NS) * 2 + 1) * kStreamTPB + threadIdx.x], prm.filter + (uint64_t)shNew * 4);
-                cp_async_commit();
-                sb[(J + LA) % NS] = start;
-                laInv = invN;
-                laPrev = shNew;
-            } else if constexpr (LA > 0) {
-                if (SBF_Q_PF != 0 && shNew != laPrev) prefetch_shard(prm.filter + (uint64_t)shNew * 4);
-                laPrev = shNew;
-                sh = kq[J % LA];
-                kq[J % LA] = shNew;
-            }
-            // a4: the newest s-mer of k-mer p
-            uint64_t Mn[NW];
-            expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
-            // a1: validity of k-mer p
-            const bool inval = (__funnelshift_r(glo, ghi, J) & maskL) != 0;
-            if constexpr (INSERT) {
+        for (int q = 0; q < NW; ++q) acc[q] = 0;
+        uint32_t prevShard = 0;
+        bool prevInval = true;
+        for (int b = 0; b < prm.chunk_blocks; ++b) {
+            const uint32_t wnext = __ldg(pw + b + 4);
+            const uint32_t v16 = __ldg(vw + b);
+            static_for<0, 16>([&](auto jc) {
+                constexpr int J = decltype(jc)::value;
+                // a2/a3: key of the newest m-mer of k-mer p = p0+16b+J, its window minimum, its shard
+                const uint32_t sh = sigma32(smin.template push<J + WN - 1>(g_key(lmer<J + WN - 1, M>(W), M)), prm.shard_shift);
+                // a4: the newest s-mer of k-mer p
+                uint64_t Mn[NW];
+                expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
+                // a1: validity of k-mer p
+                const bool inval = (v16 & (1u << J)) != 0;
                 const bool brk = (sh != prevShard) || (inval != prevInval);
                 if (brk) {
                     if (!prevInval) { // a5: flush the finished run
@@ -516,106 +627,66 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
                 for (int q = 0; q < NW; ++q) acc[q] |= Mn[q];
                 prevShard = sh;
                 prevInval = inval;
-            } else {
-                if constexpr (STAGE) {
-                    if (sb[J % NS]) { // a6: the run starting here: its shard was staged LA positions ago
-                        cp_async_wait<LA>();
-                        const uint4 lo = stage[((J % NS) * 2) * kStreamTPB + threadIdx.x];
-                        const uint4 hi = stage[((J % NS) * 2 + 1) * kStreamTPB + threadIdx.x];
-                        shard[0] = ((uint64_t)lo.y << 32) | lo.x; shard[1] = ((uint64_t)lo.w << 32) | lo.z;
-                        shard[2] = ((uint64_t)hi.y << 32) | hi.x; shard[3] = ((uint64_t)hi.w << 32) | hi.z;
-                    }
-                } else {
-                    const bool need = !inval && (prevInval || sh != prevShard);
-                    if (need) { // a6: fetch the shard of the new run
-                        ld_shard_256(prm.filter + (uint64_t)sh * 4, shard);
-                        prevShard = sh;
-                        prevInval = false;
-                    }
-                }
-                uint64_t miss = 0;
-                if constexpr (Z == 3) {
-                    // pair ORs: PB = M[t-2]|M[t-3], PC = M[t-1]|M[t-2]; K = (Mn | M[t-1]) | PB
-                    uint64_t mq[NW];
 #pragma unroll
-                    for (int q = 0; q < NW; ++q) {
-                        const uint64_t cn = Mn[q] | Mh[(J + 2) % RZ][q];
-                        mq[q] = (cn | PB[q]) & ~shard[q];
-                        PB[q] = PC[q];
-                        PC[q] = cn;
-                    }
-                    if constexpr (NW == 4) miss = (mq[0] | mq[1] | mq[2]) | mq[3];
-                    else
+                for (int q = 0; q < NW; ++q) Mh[(J + Z) % RZ][q] = Mn[q];
+            });
+            W[0] = W[1]; W[1] = W[2]; W[2] = W[3]; W[3] = wnext;
+        }
+        if (!prevInval) {
+            uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
 #pragma unroll
-                        for (int q = 0; q < NW; ++q) miss |= mq[q];
-                } else {
-#pragma unroll
-                    for (int q = 0; q < NW; ++q) {
-                        uint64_t kq_ = Mn[q];
-#pragma unroll
-                        for (int i = 0; i < Z; ++i) kq_ |= Mh[(J + i) % RZ][q];
-                        miss |= kq_ & ~shard[q];
-                    }
-                }
-                if (!inval && miss == 0) res16 |= 1u << J;
-            }
-#pragma unroll
-            for (int q = 0; q < NW; ++q) Mh[(J + Z) % RZ][q] = Mn[q];
-        });
-        W[0] = W[1]; W[1] = W[2]; W[2] = W[3]; W[3] = wnext;
-        glo = (glo >> 16) | (ghi << 16);
-        ghi = (ghi >> 16) | (gnext << 16);
-        if constexpr (!INSERT) {
+            for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
+        }
+    } else {
+        QueryLane<K, M, S, H> ql;
+        ql.prologue(W, prm, stage);
+        uint32_t res = 0;
+        for (int b = 0; b < prm.chunk_blocks; ++b) {
+            const uint32_t wnext = __ldg(pw + b + 4);
+            const uint32_t v16 = __ldg(vw + b);
+            uint32_t res16 = 0;
+            static_for<0, 16>([&](auto jc) {
+                constexpr int J = decltype(jc)::value;
+                if (ql.template step<J>(W, prm, stage)) res16 |= 1u << J;
+            });
+            res16 &= ~v16; // a1: positions without a valid k-mer answer false
+            W[0] = W[1]; W[1] = W[2]; W[2] = W[3]; W[3] = wnext;
             res = (res >> 16) | (res16 << 16);
             if (b & 1) {
                 const uint64_t wi = (p0 >> 5) + (uint64_t)(b >> 1);
                 if (wi < prm.n_bitmap_words) prm.bitmap[wi] = res;
             }
         }
+        // the last kLA positions staged look-ahead copies nobody reads; drain them before the next chunk's prologue
+        // reuses the same staging slots (two unordered cp.async to one slot could land in either order)
+        cp_async_wait<0>();
     }
-    if constexpr (INSERT) {
-        if (!prevInval) {
-            uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
-#pragma unroll
-            for (int q = 0; q < NW; ++q) {
-                const uint64_t o = acc[q];
-                red_or_64(dst + q, o);
-            }
-        }
-    }
-    // the last LA positions of a chunk staged look-ahead copies nobody reads; drain them before the next chunk's
-    // prologue reuses the same staging slots (two unordered cp.async to one slot could land in either order)
-    if constexpr (STAGE) cp_async_wait<0>();
     } // chunk loop
 }
 
 // =============================================================================================
 // a2-a6 fused, RECORD MODE (query of short records, e.g. 150-base reads): one thread per record.
-// Same per-position arithmetic as stream_kernel<..., false> (staged shards, pair-OR masks), but the
-// thread walks exactly its record's k-mer start positions, so the K-1 tail positions of every
-// record (20 % of a 150-base read at k = 31) cost nothing, and the per-record hit count falls out of
-// the same registers.  The window is re-aligned to the record start with one funnel shift per
-// 16 symbols.  Output: the bitmap was zeroed by the caller (cudaMemsetAsync); words that lie wholly
-// inside the record are stored, the (at most two) words shared with neighbours are OR-ed in.
-// Runs only when the longest record of the batch is <= rec_limit (device flag from mark_ends_kernel);
-// otherwise every thread exits and the chunk-mode kernels, launched right after, do the work.
+// Same per-position arithmetic as the chunk-mode query (QueryLane), but the thread walks exactly its
+// record's k-mer start positions, so the K-1 tail positions of every record (20 % of a 150-base
+// read at k = 31) cost nothing, record ends need no marking, and the per-record hit count falls out
+// of the same registers.  The window is re-aligned to the record start with one funnel shift per
+// 16 symbols.  Output: pack_kernel zeroed the bitmap; words that lie wholly inside the record are
+// stored, the (at most two) words shared with neighbours are OR-ed in.
+// A record longer than rec_limit is not walked: the thread raises the fallback flag and the chunk
+// kernels, launched right after, redo the whole batch (they do nothing while the flag is clear).
 // =============================================================================================
 template <int K, int M, int S, int H>
 __global__ void __launch_bounds__(kStreamTPB, SBF_MINB_R) stream_rec_kernel(const StreamParams prm)
 {
-    constexpr int WN = K - M + 1;
-    constexpr int Z = K - S;
-    constexpr int NW = H < 4 ? H : 4;
-    constexpr int RZ = ring_size(Z);
-    constexpr int L = K > 1 ? K - 1 : 1;
-    constexpr int LA = 3, NS = 4;
-    constexpr uint32_t maskL = (L >= 32) ? 0xFFFFFFFFu : ((1u << L) - 1u);
-    __shared__ uint4 stage[NS * 2 * kStreamTPB];
+    __shared__ uint4 stage[kNS * 2 * kStreamTPB];
 
-    if (__ldg(prm.max_len) > prm.rec_limit) return;
     const uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= prm.n_rec) return;
     const uint64_t a = __ldg(prm.offsets + r), e = __ldg(prm.offsets + r + 1);
+    if (e - a > (uint64_t)prm.rec_limit) {
+        *prm.fallback = 1;
+        return;
+    }
     const uint32_t len = (uint32_t)(e - a);
     const uint32_t nk = len >= (uint32_t)K ? len - K + 1 : 0; // k-mer start positions of the record
     if (nk == 0) {
@@ -623,7 +694,7 @@ __global__ void __launch_bounds__(kStreamTPB, SBF_MINB_R) stream_rec_kernel(cons
         return;
     }
     const uint32_t *__restrict__ pw = prm.packed + (a >> 4);
-    const uint16_t *__restrict__ gw = prm.gmask + (a >> 4);
+    const uint16_t *__restrict__ vw = prm.vmask + (a >> 4);
     const uint32_t s2 = 2u * (uint32_t)(a & 15), s1 = (uint32_t)(a & 15);
     uint32_t rawLast;
     uint32_t W[kWin];
@@ -633,100 +704,10 @@ __global__ void __launch_bounds__(kStreamTPB, SBF_MINB_R) stream_rec_kernel(cons
         W[0] = __funnelshift_l(r1, r0, s2); W[1] = __funnelshift_l(r2, r1, s2);
         W[2] = __funnelshift_l(r3, r2, s2); W[3] = __funnelshift_l(rawLast, r3, s2);
     }
-    uint32_t glo, ghi, gLast; // G bits of positions a.. (bit 0 = position a), re-aligned like the window
-    {
-        const uint32_t g0 = (uint32_t)__ldg(gw) | ((uint32_t)__ldg(gw + 1) << 16);
-        const uint32_t g1 = (uint32_t)__ldg(gw + 2) | ((uint32_t)__ldg(gw + 3) << 16);
-        gLast = __ldg(gw + 4);
-        glo = __funnelshift_r(g0, g1, s1);
-        ghi = __funnelshift_r(g1, gLast, s1);
-    }
+    uint32_t vcur = (uint32_t)__ldg(vw) | ((uint32_t)__ldg(vw + 1) << 16); // V bits of the symbols from 16*(a>>4) on
 
-    SlidingMin<WN> smin;
-#pragma unroll
-    for (int i = 0; i < 16; ++i) { smin.g[i] = 0; smin.c3[i] = 0; smin.c9[i] = 0; }
-    uint64_t Mh[RZ][NW];
-#pragma unroll
-    for (int i = 0; i < RZ; ++i)
-#pragma unroll
-        for (int q = 0; q < NW; ++q) Mh[i][q] = 0;
-    static_for<0, WN - 1>([&](auto ec) {
-        constexpr int E = decltype(ec)::value;
-        (void)smin.template push<E>(g_key(lmer<E, M>(W), M));
-    });
-    static_for<0, Z>([&](auto ic) {
-        constexpr int I = decltype(ic)::value;
-        expand_masks<H, NW>(f_hash_c<S>(lmer<I, S>(W)), Mh[I % RZ]);
-    });
-    uint64_t PB[NW], PC[NW];
-#pragma unroll
-    for (int q = 0; q < NW; ++q) {
-        PB[q] = Mh[0][q] | Mh[1 % RZ][q];
-        PC[q] = Mh[1 % RZ][q] | Mh[2 % RZ][q];
-    }
-    uint32_t laPrev = 0xFFFFFFFFu;
-    bool sb[NS], laInv = true;
-#pragma unroll
-    for (int i = 0; i < NS; ++i) sb[i] = false;
-    uint64_t shard[4] = {0, 0, 0, 0};
-
-    // lookahead stage for k-mer q = (block start) + QJ: shard index, run start -> stage the sector
-    auto look = [&](auto qc) {
-        constexpr int QJ = decltype(qc)::value; // 0 .. 15+LA relative to the current window
-        const uint32_t shNew = sigma32(smin.template push<QJ + WN - 1>(g_key(lmer<QJ + WN - 1, M>(W), M)), prm.shard_shift);
-        const bool invN = (__funnelshift_r(glo, ghi, QJ) & maskL) != 0;
-        const bool start = !invN && (laInv || shNew != laPrev);
-        if (start)
-            cp_async_shard(&stage[((QJ % NS) * 2) * kStreamTPB + threadIdx.x], &stage[((QJ % NS) * 2 + 1) * kStreamTPB + threadIdx.x],
-                           prm.filter + (uint64_t)shNew * 4);
-        cp_async_commit();
-        sb[QJ % NS] = start;
-        laInv = invN;
-        laPrev = shNew;
-    };
-    static_for<0, LA>(look);
-
-    uint32_t res16 = 0;
-    auto step = [&](auto jc) {
-        constexpr int J = decltype(jc)::value;
-        look(std::integral_constant<int, J + LA>{});
-        uint64_t Mn[NW];
-        expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
-        const bool inval = (__funnelshift_r(glo, ghi, J) & maskL) != 0;
-        if (sb[J % NS]) {
-            cp_async_wait<LA>();
-            const uint4 lo = stage[((J % NS) * 2) * kStreamTPB + threadIdx.x];
-            const uint4 hi = stage[((J % NS) * 2 + 1) * kStreamTPB + threadIdx.x];
-            shard[0] = ((uint64_t)lo.y << 32) | lo.x; shard[1] = ((uint64_t)lo.w << 32) | lo.z;
-            shard[2] = ((uint64_t)hi.y << 32) | hi.x; shard[3] = ((uint64_t)hi.w << 32) | hi.z;
-        }
-        uint64_t miss = 0;
-        if constexpr (Z == 3) {
-            uint64_t mq[NW];
-#pragma unroll
-            for (int q = 0; q < NW; ++q) {
-                const uint64_t cn = Mn[q] | Mh[(J + 2) % RZ][q];
-                mq[q] = (cn | PB[q]) & ~shard[q];
-                PB[q] = PC[q];
-                PC[q] = cn;
-            }
-            if constexpr (NW == 4) miss = (mq[0] | mq[1] | mq[2]) | mq[3];
-            else
-#pragma unroll
-                for (int q = 0; q < NW; ++q) miss |= mq[q];
-        } else {
-#pragma unroll
-            for (int q = 0; q < NW; ++q) {
-                uint64_t kq_ = Mn[q];
-#pragma unroll
-                for (int i = 0; i < Z; ++i) kq_ |= Mh[(J + i) % RZ][q];
-                miss |= kq_ & ~shard[q];
-            }
-        }
-        if (!inval && miss == 0) res16 |= 1u << J;
-#pragma unroll
-        for (int q = 0; q < NW; ++q) Mh[(J + Z) % RZ][q] = Mn[q];
-    };
+    QueryLane<K, M, S, H> ql;
+    ql.prologue(W, prm, stage);
 
     // result bits leave through a 64-bit buffer aligned to the bitmap's words
     uint64_t rb = 0;
@@ -746,17 +727,21 @@ __global__ void __launch_bounds__(kStreamTPB, SBF_MINB_R) stream_rec_kernel(cons
     const uint32_t nblk = (nk + 15) >> 4;
     for (uint32_t b = 0; b < nblk; ++b) {
         const uint32_t rawNext = __ldg(pw + b + 5);
-        const uint32_t gNext = __ldg(gw + b + 5);
-        res16 = 0;
-        static_for<0, 8>(step);
-        if (16 * b + 8 < nk) static_for<8, 16>(step);
+        const uint32_t vNext = __ldg(vw + b + 2);
+        uint32_t res16 = 0;
+        static_for<0, 8>([&](auto jc) {
+            constexpr int J = decltype(jc)::value;
+            if (ql.template step<J>(W, prm, stage)) res16 |= 1u << J;
+        });
+        if (16 * b + 8 < nk)
+            static_for<8, 16>([&](auto jc) {
+                constexpr int J = decltype(jc)::value;
+                if (ql.template step<J>(W, prm, stage)) res16 |= 1u << J;
+            });
         W[0] = W[1]; W[1] = W[2]; W[2] = W[3]; W[3] = __funnelshift_l(rawNext, rawLast, s2);
         rawLast = rawNext;
-        // next 16 re-aligned G bits = bits [s1, s1+16) of gLast | gNext << 16
-        const uint32_t g16 = (__funnelshift_r(gLast | (gNext << 16), 0u, s1)) & 0xFFFFu;
-        glo = (glo >> 16) | (ghi << 16);
-        ghi = (ghi >> 16) | (g16 << 16);
-        gLast = gNext;
+        res16 &= ~(vcur >> s1) & 0xFFFFu;   // a1: V bits of these 16 positions (re-aligned like the window)
+        vcur = (vcur >> 16) | (vNext << 16);
         if (16 * b + 16 > nk) res16 &= (1u << (nk - 16 * b)) - 1u; // positions past the record's last k-mer
         cnt += __popc(res16);
         rb |= (uint64_t)res16 << fill;
@@ -788,12 +773,9 @@ __device__ __forceinline__ uint64_t load_kmer(const uint32_t *__restrict__ packe
     return v >> (64 - 2 * k);
 }
 
-__device__ __forceinline__ bool kmer_invalid(const uint16_t *__restrict__ gmask, uint64_t p, int k)
+__device__ __forceinline__ bool kmer_invalid(const uint16_t *__restrict__ vmask, uint64_t p)
 {
-    const uint16_t *g = gmask + (p >> 4);
-    uint64_t bits = (uint64_t)__ldg(g) | ((uint64_t)__ldg(g + 1) << 16) | ((uint64_t)__ldg(g + 2) << 32);
-    int L = k > 1 ? k - 1 : 1;
-    return ((bits >> (p & 15)) & low_mask64(L)) != 0;
+    return ((__ldg(vmask + (p >> 4)) >> (p & 15)) & 1u) != 0;
 }
 
 template <bool INSERT>
@@ -803,7 +785,7 @@ __global__ void __launch_bounds__(256) naive_kernel(const NaiveParams np)
     const int k = np.k, m = np.m, s = np.s, H = np.H;
     const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; // grid covers a multiple of 32 positions
     bool present = false;
-    if (p < prm.n_pos && !kmer_invalid(prm.gmask, p, k)) {
+    if (p < prm.n_pos && !kmer_invalid(prm.vmask, p)) {
         const uint64_t v = load_kmer(prm.packed, p, k);
         uint32_t minKey = 0xFFFFFFFFu;
         for (int i = 0; i <= k - m; ++i) { // Alg. 1 l.5-9
@@ -864,9 +846,9 @@ __device__ __forceinline__ uint32_t popc_range(const uint32_t *__restrict__ bm, 
 // short records: one thread per record
 __global__ void __launch_bounds__(256) count_records_thread_kernel(const uint32_t *__restrict__ bm, const uint64_t *__restrict__ offsets,
                                                                    uint64_t n_rec, uint32_t *__restrict__ counts,
-                                                                   const uint32_t *max_len, uint32_t rec_limit)
+                                                                   const uint32_t *only_if)
 {
-    if (max_len != nullptr && __ldg(max_len) <= rec_limit) return; // stream_rec_kernel wrote the counts
+    if (only_if != nullptr && *only_if == 0) return; // stream_rec_kernel wrote the counts
     for (uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; r < n_rec; r += (uint64_t)gridDim.x * blockDim.x)
         counts[r] = popc_range(bm, offsets[r], offsets[r + 1]);
 }

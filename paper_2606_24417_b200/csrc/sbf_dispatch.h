@@ -24,7 +24,7 @@ cudaError_t launch_stream(const StreamParams &prm, cudaStream_t stream)
     const uint64_t chunks = (prm.n_pos + per - 1) / per;
     if (chunks == 0) return cudaSuccess;
     uint64_t blocks = (chunks + kStreamTPB - 1) / kStreamTPB;
-    if (!INSERT && prm.max_len != nullptr && blocks > 148 * 8) blocks = 148 * 8; // fallback behind record mode: strides
+    if (!INSERT && prm.fallback != nullptr && blocks > 148 * 8) blocks = 148 * 8; // fallback behind record mode: strides
     stream_kernel<K, M, S, H, INSERT><<<(unsigned)blocks, kStreamTPB, 0, stream>>>(prm);
     return cudaGetLastError();
 }

@@ -307,7 +307,7 @@ def test_host_facing_calls_match_device_facing():
 
 
 def test_pack_kernel_words_and_mask():
-    """a1 on its own: packed 2-bit words and the validity mask against a plain numpy restatement."""
+    """a1 on its own: packed 2-bit words and the k-mer validity bits V against a plain numpy restatement."""
     rng = np.random.default_rng(3)
     seq = seqgen.uniform(51, 5000)
     seq[rng.integers(0, seq.size, 60)] = ord("N")
@@ -328,8 +328,11 @@ def test_pack_kernel_words_and_mask():
         want_valid_words |= cc[:, j].astype(np.uint64) << np.uint64(30 - 2 * j)
     ok_word = ~inv[: 16 * nw].reshape(nw, 16).any(axis=1)
     assert np.array_equal(words[ok_word], want_valid_words[ok_word].astype(np.uint32))
-    G = inv[:-1] | inv[1:]
-    want_mask = (G.reshape(nw, 16) << np.arange(16)).sum(axis=1).astype(np.uint16)
+    # V[j] = some symbol of [j, j+k) is not ACGT or lies past the end: no valid k-mer starts at j
+    ext = np.concatenate((inv, np.ones(k, bool)))
+    cs = np.concatenate(([0], np.cumsum(ext)))
+    V = (cs[k:k + 16 * nw] - cs[:16 * nw]) > 0
+    want_mask = (V.reshape(nw, 16) << np.arange(16)).sum(axis=1).astype(np.uint16)
     assert np.array_equal(mask, want_mask)
 
 
