@@ -20,6 +20,13 @@ namespace {
 
 constexpr uint64_t kHostChunkDefault = 32ull << 20; // host-facing path: symbols per staged chunk, multiple of 128 (measured best of 8..128 Mi)
 
+// insert: from this filter size on a run is flushed with one 32-byte TMA reduction instead of four RED.OR.B64
+// (measured per 100 Mbp on B200: 2^31 bits 0.48 vs 0.50 ms, 2^32 bits 0.49 vs 0.57 ms, 2^35 bits 0.58 vs 0.70 ms; 2^30 bits 0.48 vs 0.38 ms)
+#ifndef SBF_TMA_MIN_BYTES
+#define SBF_TMA_MIN_BYTES (256ull << 20)
+#endif
+constexpr uint64_t kTmaFlushMinBytes = SBF_TMA_MIN_BYTES;
+
 thread_local std::string g_err;
 std::atomic<uint64_t> g_launches{0};
 
@@ -111,6 +118,7 @@ struct sbf {
     uint64_t num_shards;
     uint64_t *filter;        // 4 * num_shards words
     const KernelEntry *entry; // nullptr -> runtime-parameter kernels
+    bool tma_flush;           // insert flushes runs with TMA reductions (filter much larger than L2)
     // scratch of the last batch
     uint32_t *packed;
     uint16_t *gmask;
@@ -217,7 +225,7 @@ int run_main(sbf *f, uint64_t total, uint32_t *bitmap, cudaStream_t st)
     if (total == 0) return SBF_OK;
     StreamParams p = make_params(f, total, bitmap);
     if (f->entry) {
-        CK((INSERT ? f->entry->insert : f->entry->query)(p, st));
+        CK((INSERT ? (f->tma_flush ? f->entry->insert_tma : f->entry->insert) : f->entry->query)(p, st));
     } else {
         NaiveParams np;
         np.sp = p; np.k = f->k; np.m = f->m; np.s = f->s; np.H = f->H;
@@ -363,6 +371,7 @@ sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits)
     f->k = k; f->m = m; f->s = s; f->H = H; f->P = P; f->device = dev;
     f->num_shards = shards;
     f->host_chunk = kHostChunkDefault;
+    f->tma_flush = shards * 32 >= kTmaFlushMinBytes;
     f->entry = P < 32 ? find_entry(k, m, s, H) : nullptr; // the specialised kernels take sigma's shift as a multiply by 2^P
     e = cudaMalloc(&f->filter, shards * 32);
     if (e == cudaSuccess) e = cudaMemset(f->filter, 0, shards * 32);

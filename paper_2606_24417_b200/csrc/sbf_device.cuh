@@ -140,6 +140,23 @@ __device__ __forceinline__ void red_or_64(uint64_t *p, uint64_t v)
     asm volatile("red.global.or.b64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
+// One sector update as a single 32-byte TMA reduction (SASS UBLKRED): the four words go to a shared-memory slot of
+// this thread and one cp.reduce.async.bulk ORs them into the filter.  Two slots per thread: before a slot is rewritten
+// the bulk operation that read it two flushes ago must have finished reading (wait_group.read 1).
+constexpr int kFlushSlots = 2;
+__device__ __forceinline__ void tma_or_sector(uint64_t *dst, const uint64_t (&w)[4], ulonglong2 *slots, uint32_t &n_flushed)
+{
+    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(kFlushSlots - 1) : "memory");
+    ulonglong2 *s = slots + ((n_flushed & (kFlushSlots - 1)) * kStreamTPB + threadIdx.x) * 2; // [slot][thread][2 x 16 bytes]
+    s[0] = make_ulonglong2(w[0], w[1]);
+    s[1] = make_ulonglong2(w[2], w[3]);
+    ++n_flushed;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(s);
+    asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.or.b64 [%0], [%1], 32;" ::"l"(dst), "r"(a0) : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+
 // =============================================================================================
 // a1: pack.  Thread i produces packed words 2i, 2i+1 and the 32 V bits of symbols [32i, 32i+32).
 //   code: A=0 C=1 G=2 T=3 (either case, A9); anything else is invalid (code bits arbitrary).
@@ -210,9 +227,15 @@ __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ s
         word[w >> 2] |= c8 << (24 - 8 * (w & 3));
         inv |= i4 << (4 * w);
     }
-    // B of the next 32 symbols: the next lane's word, or (last lane of the warp) classified here
-    uint32_t nxt = __shfl_down_sync(0xFFFFFFFFu, inv, 1);
-    if ((threadIdx.x & 31) == 31) {
+    // B of the next 32 symbols: the next thread's word through shared memory; only the last thread of the CTA has to
+    // classify them itself (a per-warp exchange would send one lane in 32 down that divergent path)
+    __shared__ uint32_t s_inv[256];
+    s_inv[threadIdx.x] = inv;
+    __syncthreads();
+    uint32_t nxt;
+    if (threadIdx.x + 1 < blockDim.x) {
+        nxt = s_inv[threadIdx.x + 1];
+    } else {
         load32(seq, b0 + 32, len, aligned16, v);
         nxt = 0;
 #pragma unroll
@@ -551,9 +574,15 @@ struct QueryLane {
 // Each m-mer key and each s-mer hash is computed once per position (not once per k-mer as in
 // Alg. 1/2); the result bits are the same because OR/AND do not care about order or repetition.
 // =============================================================================================
-template <int K, int M, int S, int H, bool INSERT>
-__global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) stream_kernel(const StreamParams prm)
+// MODE: kModeQuery, kModeInsert (flush = four RED.OR.B64), kModeInsertTma (flush = one 32-byte TMA reduction: faster
+// once the filter is much larger than L2 — the LSU path then spends four L2 requests on a sector that one DRAM
+// read-modify-write serves; slower while the filter is L2-resident, where the TMA unit's ~24 G operations/s cap binds).
+constexpr int kModeQuery = 0, kModeInsert = 1, kModeInsertTma = 2;
+template <int K, int M, int S, int H, int MODE>
+__global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : SBF_MINB_Q) stream_kernel(const StreamParams prm)
 {
+    constexpr bool INSERT = MODE != kModeQuery;
+    constexpr bool TMA_FLUSH = MODE == kModeInsertTma;
     constexpr int WN = K - M + 1;
     constexpr int Z = K - S;
     constexpr int NW = H < 4 ? H : 4;
@@ -561,6 +590,9 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
     static_assert(K >= 1 && K <= 32 && M >= 1 && M <= K && S >= 1 && S <= K, "bad k/m/s");
     static_assert(Z <= 16, "stream kernel supports k-s <= 16");
     __shared__ uint4 stage[INSERT ? 1 : kNS * 2 * kStreamTPB];
+    __shared__ ulonglong2 flush_slots[TMA_FLUSH ? kFlushSlots * kStreamTPB * 2 : 1];
+    uint32_t n_flushed = 0;
+    (void)flush_slots; (void)n_flushed;
 
     if constexpr (!INSERT) {
         if (prm.fallback != nullptr && *prm.fallback == 0) return; // stream_rec_kernel did this batch
@@ -612,8 +644,14 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
                 if (brk) {
                     if (!prevInval) { // a5: flush the finished run
                         uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
+                        if constexpr (TMA_FLUSH) {
+                            const uint64_t w4[4] = {acc[0], NW > 1 ? acc[NW > 1 ? 1 : 0] : 0, NW > 2 ? acc[NW > 2 ? 2 : 0] : 0,
+                                                    NW > 3 ? acc[NW > 3 ? 3 : 0] : 0};
+                            tma_or_sector(dst, w4, flush_slots, n_flushed);
+                        } else {
 #pragma unroll
-                        for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
+                            for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
+                        }
                     }
 #pragma unroll
                     for (int q = 0; q < NW; ++q) { // restart with the k-s s-mers shared with the previous k-mers
@@ -634,9 +672,16 @@ __global__ void __launch_bounds__(kStreamTPB, INSERT ? SBF_MINB_I : SBF_MINB_Q) 
         }
         if (!prevInval) {
             uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
+            if constexpr (TMA_FLUSH) {
+                const uint64_t w4[4] = {acc[0], NW > 1 ? acc[NW > 1 ? 1 : 0] : 0, NW > 2 ? acc[NW > 2 ? 2 : 0] : 0,
+                                        NW > 3 ? acc[NW > 3 ? 3 : 0] : 0};
+                tma_or_sector(dst, w4, flush_slots, n_flushed);
+            } else {
 #pragma unroll
-            for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
+                for (int q = 0; q < NW; ++q) red_or_64(dst + q, acc[q]);
+            }
         }
+        if constexpr (TMA_FLUSH) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); // slots intact until read
     } else {
         QueryLane<K, M, S, H> ql;
         ql.prologue(W, prm, stage);

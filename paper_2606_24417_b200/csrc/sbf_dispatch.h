@@ -12,20 +12,22 @@ typedef cudaError_t (*stream_launch_fn)(const StreamParams &prm, cudaStream_t st
 
 struct KernelEntry {
     int k, m, s, H;
-    stream_launch_fn insert;
+    stream_launch_fn insert;     // run flush = four RED.OR.B64
+    stream_launch_fn insert_tma; // run flush = one 32-byte TMA reduction (filters much larger than L2)
     stream_launch_fn query;
     stream_launch_fn query_rec; // record mode (one thread per record)
 };
 
-template <int K, int M, int S, int H, bool INSERT>
+template <int K, int M, int S, int H, int MODE>
 cudaError_t launch_stream(const StreamParams &prm, cudaStream_t stream)
 {
+    constexpr bool INSERT = MODE != kModeQuery;
     const uint64_t per = 16ull * (uint64_t)prm.chunk_blocks;
     const uint64_t chunks = (prm.n_pos + per - 1) / per;
     if (chunks == 0) return cudaSuccess;
     uint64_t blocks = (chunks + kStreamTPB - 1) / kStreamTPB;
     if (!INSERT && prm.fallback != nullptr && blocks > 148 * 8) blocks = 148 * 8; // fallback behind record mode: strides
-    stream_kernel<K, M, S, H, INSERT><<<(unsigned)blocks, kStreamTPB, 0, stream>>>(prm);
+    stream_kernel<K, M, S, H, MODE><<<(unsigned)blocks, kStreamTPB, 0, stream>>>(prm);
     return cudaGetLastError();
 }
 
@@ -39,7 +41,8 @@ cudaError_t launch_stream_rec(const StreamParams &prm, cudaStream_t stream)
 }
 
 #define SBF_ENTRY(K, M, S, H) \
-    { K, M, S, H, &sbfk::launch_stream<K, M, S, H, true>, &sbfk::launch_stream<K, M, S, H, false>, \
+    { K, M, S, H, &sbfk::launch_stream<K, M, S, H, sbfk::kModeInsert>, &sbfk::launch_stream<K, M, S, H, sbfk::kModeInsertTma>, \
+      &sbfk::launch_stream<K, M, S, H, sbfk::kModeQuery>, \
       &sbfk::launch_stream_rec<K, M, S, H> }
 
 // One table per translation unit (compiled in parallel); each registers itself when the library is loaded.

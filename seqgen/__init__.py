@@ -118,6 +118,43 @@ def num_threads() -> int:
     return int(_load().sg_num_threads())
 
 
+# ---- device-side generator (seqgen_cuda.cu): the uniform stream produced on the GPU -------------------------
+_CU_SRC = os.path.join(_HERE, "seqgen_cuda.cu")
+_CU_LIB = os.path.join(_HERE, "libseqgen_cuda.so")
+_cu_lib = None
+
+
+def build_cuda(force: bool = False) -> str:
+    """Compile seqgen_cuda.cu -> libseqgen_cuda.so for sm_100a (nvcc cross-compiles without a GPU)."""
+    if force or not os.path.exists(_CU_LIB) or os.path.getmtime(_CU_LIB) < os.path.getmtime(_CU_SRC):
+        nvcc = "/usr/local/cuda/bin/nvcc" if os.path.exists("/usr/local/cuda/bin/nvcc") else "nvcc"
+        tmp = _CU_LIB + ".tmp.%d" % os.getpid()
+        subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-shared",
+                               "-Xcompiler", "-fPIC", "-o", tmp, _CU_SRC])
+        os.replace(tmp, _CU_LIB)
+    return _CU_LIB
+
+
+def uniform_device(seed: int, first: int, n: int, out=None, stream=None):
+    """Symbols [first, first + n) of the uniform(seed, .) stream as a CUDA uint8 tensor, generated on the device
+    (byte-identical to uniform(seed, first + n)[first:])."""
+    import torch
+    global _cu_lib
+    if _cu_lib is None:
+        _cu_lib = ctypes.CDLL(build_cuda())
+        _cu_lib.sg_uniform_device.restype = ctypes.c_int
+        _cu_lib.sg_uniform_device.argtypes = [ctypes.c_uint64, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_uint64,
+                                              ctypes.c_void_p]
+    if out is None:
+        out = torch.empty(n, dtype=torch.uint8, device="cuda")
+    assert out.is_cuda and out.dtype == torch.uint8 and out.numel() >= n and out.is_contiguous()
+    st = None if stream is None else stream.cuda_stream
+    rc = _cu_lib.sg_uniform_device(seed, out.data_ptr(), first, n, st)
+    if rc != 0:
+        raise RuntimeError("sg_uniform_device: CUDA error %d" % rc)
+    return out
+
+
 def fixed_offsets(n_reads: int, read_len: int, first: int = 0) -> np.ndarray:
     """offsets[n_reads+1] of back-to-back fixed-length records (relative to the batch)."""
     return (np.arange(n_reads + 1, dtype=np.uint64) * np.uint64(read_len))
