@@ -56,6 +56,17 @@ def lib():
         fn = getattr(L, name); fn.restype = u64; fn.argtypes = [p, p, p, u64, p, p]
     L.sbfo_trace_records.restype = u64; L.sbfo_trace_records.argtypes = [p, p, p, u64, p, p, p]
     L.sbfo_num_threads.restype = i32
+    # wide path (A19-A22)
+    L.sbfo_create_ex.restype = p; L.sbfo_create_ex.argtypes = [i32, i32, i32, i32, u64, i32]
+    L.sbfo_force_wide.argtypes = [p, i32]
+    L.sbfo_symbol_code.restype = i32; L.sbfo_symbol_code.argtypes = [i32, p]
+    L.sbfo_fold64.restype = u64; L.sbfo_fold64.argtypes = [u64, u64]
+    L.sbfo_pack_kmer_w.restype = i32; L.sbfo_pack_kmer_w.argtypes = [p, p, u64, u64, ctypes.POINTER(u64), ctypes.POINTER(u64)]
+    L.sbfo_sub_w.restype = u64; L.sbfo_sub_w.argtypes = [p, u64, u64, i32, i32]
+    L.sbfo_min_key_w.restype = u32; L.sbfo_min_key_w.argtypes = [p, u64, u64]
+    L.sbfo_shard_of_w.restype = u64; L.sbfo_shard_of_w.argtypes = [p, u64, u64]
+    L.sbfo_insert_kmer_w.argtypes = [p, u64, u64]
+    L.sbfo_contains_kmer_w.restype = i32; L.sbfo_contains_kmer_w.argtypes = [p, u64, u64]
     _lib = L
     return L
 
@@ -79,12 +90,13 @@ def _as_offsets(offsets, total) -> np.ndarray:
 class OracleSBF:
     """The oracle's filter object; mirrors the C-ABI names of the product for readability only."""
 
-    def __init__(self, k: int, m: int, s: int, H: int, num_bits: int):
+    def __init__(self, k: int, m: int, s: int, H: int, num_bits: int, alphabet: int = 0):
         self._L = lib()
-        self._h = self._L.sbfo_create(k, m, s, H, num_bits)
+        self._h = (self._L.sbfo_create(k, m, s, H, num_bits) if alphabet == 0 and k <= 32 else
+                   self._L.sbfo_create_ex(k, m, s, H, num_bits, alphabet))
         if not self._h:
-            raise ValueError("oracle: invalid parameters k=%d m=%d s=%d H=%d num_bits=%d" % (k, m, s, H, num_bits))
-        self.k, self.m, self.s, self.H = k, m, s, H
+            raise ValueError("oracle: invalid parameters k=%d m=%d s=%d H=%d num_bits=%d alphabet=%d" % (k, m, s, H, num_bits, alphabet))
+        self.k, self.m, self.s, self.H, self.alphabet = k, m, s, H, alphabet
         self.num_shards = int(self._L.sbfo_num_shards(self._h))
 
     def close(self):
@@ -161,6 +173,42 @@ class OracleSBF:
 
     def contains_kmer(self, v: int) -> bool:
         return bool(self._L.sbfo_contains_kmer(self._h, v))
+
+    # ---- wide path: a packed k-mer is a Python int below 2^128 ----
+    def force_wide(self, on: bool = True):
+        self._L.sbfo_force_wide(self._h, 1 if on else 0)
+
+    def pack_kmer_w(self, rec, p: int):
+        b = _as_bases(rec); hi, lo = ctypes.c_uint64(0), ctypes.c_uint64(0)
+        ok = self._L.sbfo_pack_kmer_w(self._h, _ptr(b), b.size, p, ctypes.byref(hi), ctypes.byref(lo))
+        return ((int(hi.value) << 64) | int(lo.value)) if ok else None
+
+    def sub_w(self, v: int, i: int, ln: int) -> int:
+        return int(self._L.sbfo_sub_w(self._h, v >> 64, v & _M64, i, ln))
+
+    def min_key_w(self, v: int) -> int:
+        return int(self._L.sbfo_min_key_w(self._h, v >> 64, v & _M64))
+
+    def shard_of_w(self, v: int) -> int:
+        return int(self._L.sbfo_shard_of_w(self._h, v >> 64, v & _M64))
+
+    def insert_kmer_w(self, v: int):
+        self._L.sbfo_insert_kmer_w(self._h, v >> 64, v & _M64)
+
+    def contains_kmer_w(self, v: int) -> bool:
+        return bool(self._L.sbfo_contains_kmer_w(self._h, v >> 64, v & _M64))
+
+
+_M64 = (1 << 64) - 1
+DNA, PROTEIN, TRIPLET = 0, 1, 2
+
+
+def fold64(hi, lo): return int(lib().sbfo_fold64(hi, lo))
+
+
+def symbol_code(alphabet, sym: bytes) -> int:
+    b = np.frombuffer(bytes(sym) + b"\0\0", dtype=np.uint8).copy()
+    return int(lib().sbfo_symbol_code(alphabet, _ptr(b)))
 
 
 def g(m, x): return int(lib().sbfo_g(m, x))

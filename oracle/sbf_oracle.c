@@ -86,6 +86,7 @@ sbfo_t *sbfo_create(int k, int m, int s, int H, uint64_t num_bits)
     sbfo_t *f = (sbfo_t *)calloc(1, sizeof(*f));
     if (!f) return NULL;
     f->k = k; f->m = m; f->s = s; f->H = H; f->P = P; f->num_shards = shards;
+    f->alphabet = SBFO_DNA; f->sym_bits = 2; f->sym_bytes = 1; f->wide = 0;
     f->words = (uint64_t *)calloc(shards * 4, sizeof(uint64_t));
     if (!f->words) { free(f); return NULL; }
     return f;
@@ -166,8 +167,14 @@ int sbfo_contains_kmer(const sbfo_t *f, uint64_t v)
 }
 
 /* Records are independent; no k-mer spans two records (A11). */
+static uint64_t wide_insert_records(sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec, int mt);
+static uint64_t wide_query_records(const sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec,
+                                   uint32_t *bitmap, uint32_t *hit_counts, int mt);
+static uint64_t wide_count_valid(const sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec);
+
 uint64_t sbfo_insert_records(sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec)
 {
+    if (f->wide) return wide_insert_records(f, bases, offsets, n_rec, 0);
     uint64_t n_valid = 0;
     for (uint64_t r = 0; r < n_rec; ++r) {
         const uint8_t *rec = bases + offsets[r];
@@ -183,6 +190,7 @@ uint64_t sbfo_insert_records(sbfo_t *f, const uint8_t *bases, const uint64_t *of
 uint64_t sbfo_query_records(const sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec,
                             uint32_t *bitmap, uint32_t *hit_counts)
 {
+    if (f->wide) return wide_query_records(f, bases, offsets, n_rec, bitmap, hit_counts, 0);
     uint64_t total = offsets[n_rec], n_valid = 0;
     memset(bitmap, 0, ((total + 31) / 32) * sizeof(uint32_t));
     for (uint64_t r = 0; r < n_rec; ++r) {
@@ -206,6 +214,7 @@ uint64_t sbfo_query_records(const sbfo_t *f, const uint8_t *bases, const uint64_
 
 uint64_t sbfo_count_valid_kmers(const sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec)
 {
+    if (f->wide) return wide_count_valid(f, bases, offsets, n_rec);
     uint64_t n_valid = 0;
     for (uint64_t r = 0; r < n_rec; ++r) {
         const uint8_t *rec = bases + offsets[r];
@@ -236,6 +245,7 @@ static uint64_t record_of(const uint64_t *offsets, uint64_t n_rec, uint64_t g)
 
 uint64_t sbfo_insert_records_mt(sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec)
 {
+    if (f->wide) return wide_insert_records(f, bases, offsets, n_rec, 1);
     uint64_t total = offsets[n_rec], n_valid = 0;
     int64_t nchunks = (int64_t)((total + MT_CHUNK - 1) / MT_CHUNK);
 #pragma omp parallel for schedule(dynamic, 1) reduction(+ : n_valid)
@@ -260,6 +270,7 @@ uint64_t sbfo_insert_records_mt(sbfo_t *f, const uint8_t *bases, const uint64_t 
 uint64_t sbfo_query_records_mt(const sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec,
                                uint32_t *bitmap, uint32_t *hit_counts)
 {
+    if (f->wide) return wide_query_records(f, bases, offsets, n_rec, bitmap, hit_counts, 1);
     uint64_t total = offsets[n_rec], n_valid = 0;
     int64_t nchunks = (int64_t)((total + MT_CHUNK - 1) / MT_CHUNK);
     memset(bitmap, 0, ((total + 31) / 32) * sizeof(uint32_t));
@@ -303,6 +314,199 @@ uint64_t sbfo_trace_records(const sbfo_t *f, const uint8_t *bases, const uint64_
             if (shard) shard[g] = ok ? sbfo_shard_of(f, v) : 0;
             n_valid += (uint64_t)ok;
         }
+    }
+    return n_valid;
+}
+
+/* ========================================================================
+ * Wide path (readings A19-A22 in DESIGN.md §3): the alphabets of P:139 and
+ * packed k-mers wider than one 64-bit word ("for DNA this is possible
+ * for k <= 32"; "wider packed representations, such as multiword").
+ * The same Alg. 1 / Alg. 2, one k-mer at a time, on a 128-bit packed value.
+ * ======================================================================== */
+typedef unsigned __int128 u128;
+
+/* A19: DNA = ACGT, either case, 2 bits.  Protein = the 26 letters, either case, 5 bits, code = letter - 'A'.
+ * DNA triplet = three consecutive DNA bases, 6 bits, code = 16 c0 + 4 c1 + c2 ("64 symbols, 6 bits, multi-byte"). */
+int sbfo_symbol_code(int alphabet, const uint8_t *p)
+{
+    if (alphabet == SBFO_DNA) return sbfo_code(p[0]);
+    if (alphabet == SBFO_PROTEIN) {
+        unsigned char c = p[0];
+        if (c >= 'a' && c <= 'z') c = (unsigned char)(c - 'a' + 'A');
+        return (c >= 'A' && c <= 'Z') ? c - 'A' : -1;
+    }
+    int c0 = sbfo_code(p[0]), c1 = sbfo_code(p[1]), c2 = sbfo_code(p[2]);
+    if (c0 < 0 || c1 < 0 || c2 < 0) return -1;
+    return 16 * c0 + 4 * c1 + c2;
+}
+
+/* A21: a window of more than 64 bits enters the (64-bit) hashes folded: lo XOR the golden-ratio multiple of hi,
+ * rotated by 32.  A window of at most 64 bits has hi = 0 and is passed through unchanged. */
+uint64_t sbfo_fold64(uint64_t hi, uint64_t lo)
+{
+    uint64_t t = hi * GOLD64;
+    return lo ^ ((t << 32) | (t >> 32));
+}
+
+sbfo_t *sbfo_create_ex(int k, int m, int s, int H, uint64_t num_bits, int alphabet)
+{
+    int bits = alphabet == SBFO_DNA ? 2 : alphabet == SBFO_PROTEIN ? 5 : alphabet == SBFO_TRIPLET ? 6 : 0;
+    if (!bits || k < 1 || k * bits > 128 || m < 1 || m > k || s < 1 || s > k || H < 1 || H > 32 || num_bits < 1) return NULL;
+    if (alphabet == SBFO_DNA && k <= 32) return sbfo_create(k, m, s, H, num_bits);
+    sbfo_t *f = sbfo_create(1, 1, 1, H, num_bits);          /* geometry (A8) as in the narrow path */
+    if (!f) return NULL;
+    f->k = k; f->m = m; f->s = s;
+    f->alphabet = alphabet; f->sym_bits = bits; f->sym_bytes = alphabet == SBFO_TRIPLET ? 3 : 1; f->wide = 1;
+    return f;
+}
+
+void sbfo_force_wide(sbfo_t *f, int on) { f->wide = on ? 1 : (f->alphabet != SBFO_DNA || f->k > 32); }
+
+/* ValidKmer + PackKmer (Alg. 1 l.3-4): shift by the symbol width and OR ("left-shift by the alphabet symbol
+ * width, OR in the new trailing symbol").  Triplet symbols sit at multiples of three bytes from the record start
+ * ("alignment padding to symbolWidth boundaries"), so a k-mer exists only at such a byte. */
+int sbfo_pack_kmer_w(const sbfo_t *f, const uint8_t *rec, uint64_t L, uint64_t p, uint64_t *hi, uint64_t *lo)
+{
+    if (p % (uint64_t)f->sym_bytes != 0) return 0;
+    if (p + (uint64_t)f->k * (uint64_t)f->sym_bytes > L) return 0;
+    u128 x = 0;
+    for (int i = 0; i < f->k; ++i) {
+        int c = sbfo_symbol_code(f->alphabet, rec + p + (uint64_t)i * (uint64_t)f->sym_bytes);
+        if (c < 0) return 0;
+        x = (x << f->sym_bits) | (u128)(unsigned)c;
+    }
+    *hi = (uint64_t)(x >> 64);
+    *lo = (uint64_t)x;
+    return 1;
+}
+
+/* Subwindow(packed, i, len): len symbols starting i symbols into the k-mer, first symbol most significant */
+uint64_t sbfo_sub_w(const sbfo_t *f, uint64_t hi, uint64_t lo, int i, int len)
+{
+    u128 v = ((u128)hi << 64) | lo;
+    int nbits = len * f->sym_bits;
+    u128 w = v >> ((f->k - len - i) * f->sym_bits);
+    if (nbits < 128) w &= (((u128)1) << nbits) - 1;
+    return sbfo_fold64((uint64_t)(w >> 64), (uint64_t)w);
+}
+
+/* g and f of a window of nbits bits (A1, A4 with the seed masked to the window width, at most 64 bits) */
+static uint32_t g_bits(int nbits, uint64_t x)
+{
+    x ^= SEED_M & low_bits(nbits);
+    uint32_t y = (uint32_t)x ^ (uint32_t)(x >> 32);
+    return y * MULT_G;
+}
+static uint64_t f_bits(int nbits, uint64_t x)
+{
+    x ^= SEED_S & low_bits(nbits);
+    uint64_t h = (x ^ (x >> 28)) * MULT_F;
+    return h ^ (h >> 32);
+}
+
+uint32_t sbfo_min_key_w(const sbfo_t *f, uint64_t hi, uint64_t lo)
+{
+    uint32_t min_hash = 0xFFFFFFFFu;
+    for (int i = 0; i <= f->k - f->m; ++i) {                         /* Alg. 1 l.5-9 */
+        uint32_t h = g_bits(f->m * f->sym_bits, sbfo_sub_w(f, hi, lo, i, f->m));
+        if (h < min_hash) min_hash = h;
+    }
+    return min_hash;
+}
+
+uint64_t sbfo_shard_of_w(const sbfo_t *f, uint64_t hi, uint64_t lo)
+{
+    return sbfo_sigma(sbfo_min_key_w(f, hi, lo), f->P);
+}
+
+static void kmer_masks_w(const sbfo_t *f, uint64_t hi, uint64_t lo, uint64_t w[4])
+{
+    w[0] = w[1] = w[2] = w[3] = 0;
+    for (int j = 0; j <= f->k - f->s; ++j) {                         /* Alg. 1 l.11-14 */
+        uint64_t s_hash = f_bits(f->s * f->sym_bits, sbfo_sub_w(f, hi, lo, j, f->s));
+        for (int i = 0; i < f->H; ++i)
+            w[i % 4] |= 1ull << sbfo_bitpos(s_hash, i, f->H);
+    }
+}
+
+void sbfo_insert_kmer_w(sbfo_t *f, uint64_t hi, uint64_t lo)
+{
+    uint64_t w[4];
+    uint64_t shard = sbfo_shard_of_w(f, hi, lo);
+    kmer_masks_w(f, hi, lo, w);
+    for (int q = 0; q < 4; ++q) f->words[shard * 4 + q] |= w[q];
+}
+
+int sbfo_contains_kmer_w(const sbfo_t *f, uint64_t hi, uint64_t lo)
+{
+    const uint64_t *words = f->words + sbfo_shard_of_w(f, hi, lo) * 4;
+    int present = 1;
+    for (int j = 0; j <= f->k - f->s; ++j) {                         /* Alg. 2 Contains */
+        uint64_t s_hash = f_bits(f->s * f->sym_bits, sbfo_sub_w(f, hi, lo, j, f->s));
+        for (int h = 0; h < f->H; ++h)
+            present = present && ((words[h % 4] >> sbfo_bitpos(s_hash, h, f->H)) & 1);
+    }
+    return present;
+}
+
+/* Record drivers of the wide path: every BYTE position p of every record is a candidate k-mer start (a triplet k-mer
+ * exists only where p is a multiple of 3); bit index of the query bitmap = global byte position (A22). */
+static uint64_t wide_insert_records(sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec, int mt)
+{
+    uint64_t n_valid = 0;
+    int64_t n = (int64_t)n_rec;
+    (void)mt;
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : n_valid) if (mt)
+    for (int64_t r = 0; r < n; ++r) {
+        const uint8_t *rec = bases + offsets[r];
+        uint64_t L = offsets[r + 1] - offsets[r];
+        for (uint64_t p = 0; p < L; ++p) {
+            uint64_t hi, lo, w[4];
+            if (!sbfo_pack_kmer_w(f, rec, L, p, &hi, &lo)) continue;
+            ++n_valid;
+            uint64_t shard = sbfo_shard_of_w(f, hi, lo);
+            kmer_masks_w(f, hi, lo, w);
+            for (int q = 0; q < 4; ++q)
+                if (w[q]) __atomic_fetch_or(&f->words[shard * 4 + q], w[q], __ATOMIC_RELAXED);
+        }
+    }
+    return n_valid;
+}
+
+static uint64_t wide_query_records(const sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec,
+                                   uint32_t *bitmap, uint32_t *hit_counts, int mt)
+{
+    uint64_t total = offsets[n_rec], n_valid = 0;
+    int64_t n = (int64_t)n_rec;
+    (void)mt;
+    memset(bitmap, 0, ((total + 31) / 32) * sizeof(uint32_t));
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : n_valid) if (mt)
+    for (int64_t r = 0; r < n; ++r) {
+        const uint8_t *rec = bases + offsets[r];
+        uint64_t L = offsets[r + 1] - offsets[r];
+        uint32_t hits = 0;
+        for (uint64_t p = 0; p < L; ++p) {
+            uint64_t hi, lo;
+            if (!sbfo_pack_kmer_w(f, rec, L, p, &hi, &lo)) continue;
+            ++n_valid;
+            if (sbfo_contains_kmer_w(f, hi, lo)) {
+                uint64_t g = offsets[r] + p;
+                __atomic_fetch_or(&bitmap[g >> 5], 1u << (g & 31), __ATOMIC_RELAXED);   /* records may share a word */
+                ++hits;
+            }
+        }
+        if (hit_counts) hit_counts[r] = hits;
+    }
+    return n_valid;
+}
+
+static uint64_t wide_count_valid(const sbfo_t *f, const uint8_t *bases, const uint64_t *offsets, uint64_t n_rec)
+{
+    uint64_t n_valid = 0;
+    for (uint64_t r = 0; r < n_rec; ++r) {
+        uint64_t L = offsets[r + 1] - offsets[r], hi, lo;
+        for (uint64_t p = 0; p < L; ++p) n_valid += (uint64_t)sbfo_pack_kmer_w(f, bases + offsets[r], L, p, &hi, &lo);
     }
     return n_valid;
 }

@@ -1,7 +1,7 @@
 """Parameter sweep of BASELINE.json config 5 and the FPR-vs-size experiment.
 
     python -m paper_2606_24417_b200.sweep [--scale 1.0] [--reads 2000000] [--points cross|axes]
-                                          [--log2-bits 32] [--sizes 28 34] [--out profiles/sweep_r01.md]
+                                          [--sizes 28 34] [--out profiles/sweep_r02.md]
 
 For every (s, m, H) point at k = 31 it creates a filter, inserts the config-3 sequence, queries one batch of
 config-3 reads, and reports insert / query G k-mers/s (CUDA events around the library calls, best of 3),
@@ -10,6 +10,7 @@ the measured FPR on the uniform-random reads (odd read index: aliens; expected t
 bits per inserted k-mer, and the Pareto set of (FPR, time).  Then the size sweep (Fig. 6 of the paper,
 P:389-397) for s in {28, 30, 31}.  Everything runs through the C ABI; the oracle is not involved
 (tests/ pins the bits; this tool only reports statistics).  Inputs: seeded synthetic (seqgen/).
+The FPR-vs-size experiment proper (10^9 random 31-mers, 2^22 .. 2^39 bits) is paper_2606_24417_b200/fpr_size.py.
 """
 from __future__ import annotations
 
@@ -100,9 +101,8 @@ def main():
     ap.add_argument("--scale", type=float, default=1.0, help="fraction of the 250 Mbp config-3 sequence")
     ap.add_argument("--reads", type=int, default=2_000_000)
     ap.add_argument("--points", default="cross", choices=["cross", "axes"])
-    ap.add_argument("--log2-bits", type=int, default=32)
-    ap.add_argument("--sizes", type=int, nargs=2, default=[28, 34])
-    ap.add_argument("--out", default=None)
+    ap.add_argument("--sizes", type=int, nargs=2, default=[28, 34], help="log2 of the smallest / largest filter size in bits")
+    ap.add_argument("--out", default=None, help="markdown summary; the full table goes to <out minus .md>.csv")
     args = ap.parse_args()
 
     import torch
@@ -120,39 +120,49 @@ def main():
     d_offs = torch.from_numpy(seqgen.fixed_offsets(args.reads, w.read_len).view(np.int64)).cuda()
     common = (d_seq, n_ins, d_reads, d_offs, args.reads, w.read_len, valid)
 
+    # BASELINE.json configs[4]: the (s, m, H) cross product at EVERY filter size 2^28 .. 2^34
     rows = []
-    for (s, m, H) in seqgen.config5_points(full_cross=(args.points == "cross")):
-        r = run_point(sbf, torch, k, m, s, H, 1 << args.log2_bits, *common)
-        r["time_ms"] = r["insert_ms"] + r["query_ms"]
-        rows.append(r)
-        print(json.dumps(r), flush=True)
-    front = set(pareto(rows))
-    sizes = []
     for lb in range(args.sizes[0], args.sizes[1] + 1):
-        for s in (28, 30, 31):
-            r = run_point(sbf, torch, k, 16, s, 4, 1 << lb, *common)
-            sizes.append(r)
+        for (s, m, H) in seqgen.config5_points(full_cross=(args.points == "cross")):
+            r = run_point(sbf, torch, k, m, s, H, 1 << lb, *common)
+            r["time_ms"] = r["insert_ms"] + r["query_ms"]
+            r["gkmers_s"] = (n_ins + int(valid.sum())) / r["time_ms"] / 1e6       # insert + query throughput of the point
+            rows.append(r)
             print(json.dumps(r), flush=True)
+    # Pareto set of (FPR, bits per k-mer, throughput): lower FPR, fewer bits, less time per pass
+    front = set(pareto(rows, keys=("fpr_random", "bits_per_kmer", "time_ms")))
 
     if args.out:
-        with open(args.out, "w") as fh:
-            fh.write("# Config 5 sweep and FPR vs filter size (k = 31, synthetic config-3 sequence and reads)\n\n")
-            fh.write("Command: `python -m paper_2606_24417_b200.sweep %s`\n\n" % " ".join(sys.argv[1:]))
-            fh.write("%d inserted k-mers, %d reads x %d (%d valid query k-mers, half of them aliens). Rates are whole library "
-                     "calls (pack + fused kernel + counts), best of 3, device-resident input. `spec` = specialised streaming "
-                     "kernels; `rt` = runtime-parameter kernel (Alg. 1/2 as printed, every k-mer recomputed).\n\n" %
-                     (n_ins, args.reads, w.read_len, int(valid.sum())))
-            fh.write("## (s, m, H) at 2^%d bits (%.1f bits per inserted k-mer)\n\n" % (args.log2_bits, rows[0]["bits_per_kmer"]))
-            fh.write("| s | m | H | kernel | insert G k-mers/s | query G k-mers/s | FPR (random reads) | hit rate (sampled reads) | Pareto (FPR, time) |\n")
-            fh.write("|---|---|---|---|---|---|---|---|---|\n")
+        base = args.out[:-3] if args.out.endswith(".md") else args.out
+        with open(base + ".csv", "w") as fh:
+            fh.write("log2_bits,bits_per_kmer,s,m,H,kernel,insert_gkmers_s,query_gkmers_s,step_gkmers_s,fpr_random,hit_sampled,pareto\n")
             for i, r in enumerate(rows):
-                fh.write("| %d | %d | %d | %s | %.1f | %.1f | %.3e | %.4f | %s |\n" % (
-                    r["s"], r["m"], r["H"], "spec" if r["specialized"] else "rt", r["insert_gkmers_s"], r["query_gkmers_s"],
-                    r["fpr_random"], r["hit_sampled"], "yes" if i in front else ""))
-            fh.write("\n## FPR vs filter size, (m, H) = (16, 4)\n\n| log2 bits | bits / k-mer | s | insert G k-mers/s | query G k-mers/s | FPR |\n|---|---|---|---|---|---|\n")
-            for r in sizes:
-                fh.write("| %d | %.2f | %d | %.1f | %.1f | %.3e |\n" % (r["log2_bits"], r["bits_per_kmer"], r["s"],
-                                                                   r["insert_gkmers_s"], r["query_gkmers_s"], r["fpr_random"]))
+                fh.write("%d,%.3f,%d,%d,%d,%s,%.2f,%.2f,%.2f,%.4e,%.5f,%d\n" % (
+                    r["log2_bits"], r["bits_per_kmer"], r["s"], r["m"], r["H"], "spec" if r["specialized"] else "rt",
+                    r["insert_gkmers_s"], r["query_gkmers_s"], r["gkmers_s"], r["fpr_random"], r["hit_sampled"], int(i in front)))
+        with open(args.out if args.out.endswith(".md") else base + ".md", "w") as fh:
+            fh.write("# BASELINE config 5: (s, m, H) cross product x filter sizes (k = 31, synthetic config-3 sequence and reads)\n\n")
+            fh.write("Command: `python -m paper_2606_24417_b200.sweep %s`\n\n" % " ".join(sys.argv[1:]))
+            fh.write("%d inserted k-mers, %d reads x %d (%d valid query k-mers, half of them aliens). %d points = %d (s, m, H) x "
+                     "filter sizes 2^%d .. 2^%d bits; all of them in `%s`. Rates are whole library calls (pack + fused kernel "
+                     "+ counts), best of 3, device-resident input; FPR = positives among the k-mers of the uniform-random reads; "
+                     "bits per k-mer = effective filter bits / inserted k-mers.\n\n" % (
+                         n_ins, args.reads, w.read_len, int(valid.sum()), len(rows),
+                         len(rows) // (args.sizes[1] - args.sizes[0] + 1), args.sizes[0], args.sizes[1], os.path.basename(base + ".csv")))
+            fh.write("## Pareto set of (FPR, bits per k-mer, throughput): %d of %d points\n\n" % (len(front), len(rows)))
+            fh.write("| log2 bits | bits / k-mer | s | m | H | insert G k-mers/s | query G k-mers/s | FPR |\n|---|---|---|---|---|---|---|---|\n")
+            for i in sorted(front, key=lambda i: (rows[i]["log2_bits"], rows[i]["fpr_random"])):
+                r = rows[i]
+                fh.write("| %d | %.2f | %d | %d | %d | %.1f | %.1f | %.3e |\n" % (
+                    r["log2_bits"], r["bits_per_kmer"], r["s"], r["m"], r["H"], r["insert_gkmers_s"], r["query_gkmers_s"], r["fpr_random"]))
+            hs = sorted({r["H"] for i, r in enumerate(rows) if i in front})
+            fh.write("\nH values on the Pareto set: %s (the paper: all Pareto points at H = 4, P:359).\n" % hs)
+            fh.write("\n## The one-factor axes through (28, 16, 4), per filter size\n\n")
+            fh.write("| log2 bits | s | m | H | insert G k-mers/s | query G k-mers/s | FPR | hit rate (sampled reads) |\n|---|---|---|---|---|---|---|---|\n")
+            for r in rows:
+                if sum((r["s"] != 28, r["m"] != 16, r["H"] != 4)) <= 1:
+                    fh.write("| %d | %d | %d | %d | %.1f | %.1f | %.3e | %.4f |\n" % (
+                        r["log2_bits"], r["s"], r["m"], r["H"], r["insert_gkmers_s"], r["query_gkmers_s"], r["fpr_random"], r["hit_sampled"]))
     return 0
 
 
