@@ -51,7 +51,7 @@ typedef enum sbf_status {
 
 /*
  * sbf_create — allocate a zeroed filter (A8).
- *   1 <= k <= 32 (one 64-bit word per packed k-mer); 1 <= m <= k; 1 <= s <= k;
+ *   1 <= k <= 64 (k <= 32: one 64-bit word per packed k-mer; larger k: see sbf_create_ex); 1 <= m <= k; 1 <= s <= k;
  *   1 <= H <= 32 (H <= 10 uses bit-slicing A5, H > 10 the salted multiply A6);
  *   num_bits >= 1.  numShards = next power of two >= ceil(num_bits/256), at most 2^32.
  *   Layout in device memory (A12): shard-major, four little-endian 64-bit sector words
@@ -61,6 +61,22 @@ typedef enum sbf_status {
  *   Returns NULL on error.
  */
 sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits);
+
+/*
+ * sbf_create_ex — the same for any of the paper's three alphabets and for packed k-mers wider than one 64-bit
+ * word ("multiword"); readings A19-A22 of DESIGN.md §3.  k * symbol_bits <= 128:
+ *   SBF_ALPHABET_DNA          2 bits, A C G T either case, k <= 64 (sbf_create is this alphabet; k <= 32 runs the
+ *                             specialised / runtime kernels above, 33 <= k <= 64 the wide kernel)
+ *   SBF_ALPHABET_PROTEIN      5 bits, the 26 letters either case (code = letter - 'A'), k <= 25
+ *   SBF_ALPHABET_DNA_TRIPLET  6 bits, one symbol = three DNA bases (code = 16 c0 + 4 c1 + c2), k <= 21; symbols sit at
+ *                             multiples of three bytes from the start of their record; k, m, s count SYMBOLS
+ * All `len` / `total_bases` / offsets stay in BYTES.  Result bitmaps are indexed by the BYTE position of a k-mer's
+ * first byte.  A window wider than 64 bits is folded (lo ^ rotl32(hi * 0x9E3779B97F4A7C15)) before it is hashed.
+ * These run one general CUDA kernel (Alg. 1/2 as printed, one k-mer per thread): correct, not tuned — the paper
+ * evaluates DNA only and calls the larger alphabets "functional".
+ */
+typedef enum sbf_alphabet { SBF_ALPHABET_DNA = 0, SBF_ALPHABET_PROTEIN = 1, SBF_ALPHABET_DNA_TRIPLET = 2 } sbf_alphabet;
+sbf_t *sbf_create_ex(int k, int m, int s, int H, uint64_t num_bits, int alphabet);
 
 /* sbf_destroy — free filter and scratch.  Synchronises the device.  NULL is ignored. */
 void sbf_destroy(sbf_t *f);

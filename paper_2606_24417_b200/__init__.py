@@ -30,6 +30,7 @@ SBF_ERR_CUDA = -4
 _u64, _u32, _i32, _p, _cp = ctypes.c_uint64, ctypes.c_uint32, ctypes.c_int, ctypes.c_void_p, ctypes.c_char_p
 ABI = {
     "sbf_create": (_p, [_i32, _i32, _i32, _i32, _u64]),
+    "sbf_create_ex": (_p, [_i32, _i32, _i32, _i32, _u64, _i32]),
     "sbf_destroy": (None, [_p]),
     "sbf_num_bits": (_u64, [_p]),
     "sbf_num_shards": (_u64, [_p]),
@@ -145,6 +146,17 @@ def sbf_create(k: int, m: int, s: int, H: int, num_bits: int) -> int:
     return h
 
 
+ALPHABET_DNA, ALPHABET_PROTEIN, ALPHABET_DNA_TRIPLET = 0, 1, 2
+
+
+def sbf_create_ex(k: int, m: int, s: int, H: int, num_bits: int, alphabet: int) -> int:
+    L = load_library()
+    h = L.sbf_create_ex(k, m, s, H, num_bits, alphabet)
+    if not h:
+        raise SBFError(SBF_ERR_INVALID_ARG, L.sbf_last_error().decode())
+    return h
+
+
 def sbf_destroy(h): load_library().sbf_destroy(h)
 def sbf_num_bits(h) -> int: return int(load_library().sbf_num_bits(h))
 def sbf_num_shards(h) -> int: return int(load_library().sbf_num_shards(h))
@@ -253,9 +265,9 @@ def sbf_debug_last_packed(h, n_words: int):
 class SuperBloomFilter:
     """Convenience owner of one handle (context manager); methods forward to the C ABI."""
 
-    def __init__(self, k: int = 31, m: int = 16, s: int = 28, H: int = 4, num_bits: int = 1 << 32):
-        self.k, self.m, self.s, self.H = k, m, s, H
-        self.handle = sbf_create(k, m, s, H, num_bits)
+    def __init__(self, k: int = 31, m: int = 16, s: int = 28, H: int = 4, num_bits: int = 1 << 32, alphabet: int = 0):
+        self.k, self.m, self.s, self.H, self.alphabet = k, m, s, H, alphabet
+        self.handle = sbf_create_ex(k, m, s, H, num_bits, alphabet)
         self.num_shards = sbf_num_shards(self.handle)
         self.num_bits = sbf_num_bits(self.handle)
         self.specialized = sbf_is_specialized(self.handle)

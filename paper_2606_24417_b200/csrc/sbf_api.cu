@@ -119,6 +119,10 @@ struct sbf {
     uint64_t *filter;        // 4 * num_shards words
     const KernelEntry *entry; // nullptr -> runtime-parameter kernels
     bool tma_flush;           // insert flushes runs with TMA reductions (filter much larger than L2)
+    // wide path (A19-A22): other alphabets, packed k-mers wider than 64 bits -> wide_kernel, no pack pass
+    int alphabet, sym_bits, sym_bytes;
+    bool wide;
+    int phase0;               // host-facing chunks only: see WideParams::phase0
     // scratch of the last batch
     uint32_t *packed;
     uint16_t *gmask;
@@ -248,10 +252,33 @@ int mark(sbf *f, int i, cudaStream_t st)
     return SBF_OK;
 }
 
+// wide path: one kernel straight from the ASCII bytes (marks 0 -> 1 -> 2 keep the timing ABI's shape: "pack" = 0)
+template <bool INSERT>
+int run_wide(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, uint32_t *bitmap,
+             cudaStream_t st)
+{
+    int rc = mark(f, 0, st);
+    if (rc) return rc;
+    rc = mark(f, 1, st);
+    if (rc) return rc;
+    WideParams p;
+    p.bases = reinterpret_cast<const uint8_t *>(d_bases); p.total = total;
+    p.offsets = (d_offsets && n_rec > 0) ? d_offsets : nullptr; p.n_rec = n_rec;
+    p.filter = f->filter; p.shard_shift = 32 - f->P; p.bitmap = bitmap; p.n_bitmap_words = (total + 31) / 32;
+    p.k = f->k; p.m = f->m; p.s = f->s; p.H = f->H; p.alphabet = f->alphabet; p.sym_bits = f->sym_bits; p.sym_bytes = f->sym_bytes;
+    p.phase0 = f->phase0;
+    const uint64_t n32 = (total + 31) / 32 * 32;
+    wide_kernel<INSERT><<<(unsigned)((n32 + 255) / 256), 256, 0, st>>>(p);
+    CK(cudaGetLastError());
+    g_launches++;
+    return mark(f, 2, st);
+}
+
 int run_insert(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, cudaStream_t st)
 {
     if (total == 0) return SBF_OK;
     apply_l2_window(f, st);
+    if (f->wide) return run_wide<true>(f, d_bases, d_offsets, n_rec, total, nullptr, st);
     int rc = mark(f, 0, st);
     if (rc) return rc;
     rc = run_pack(f, d_bases, d_offsets, n_rec, total, st);
@@ -292,6 +319,16 @@ int run_query(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n
 {
     if (total == 0) return SBF_OK;
     apply_l2_window(f, st);
+    if (f->wide) {
+        int rcw = run_wide<false>(f, d_bases, d_offsets, n_rec, total, d_bitmap, st);
+        if (rcw) return rcw;
+        if (d_counts && d_offsets && n_rec) {
+            rcw = run_count_records(d_bitmap, d_offsets, n_rec, total, d_counts, st);
+            if (rcw) return rcw;
+            rcw = mark(f, 3, st);
+        }
+        return rcw;
+    }
     const bool try_rec = f->entry && f->entry->query_rec && d_offsets && n_rec > 0 && total / n_rec <= kRecMeanLimit;
     int rc = mark(f, 0, st);
     if (rc) return rc;
@@ -343,11 +380,18 @@ extern "C" {
 const char *sbf_last_error(void) { return g_err.c_str(); }
 uint64_t sbf_kernel_launches(void) { return g_launches.load(); }
 
-sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits)
+sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits) { return sbf_create_ex(k, m, s, H, num_bits, SBF_ALPHABET_DNA); }
+
+sbf_t *sbf_create_ex(int k, int m, int s, int H, uint64_t num_bits, int alphabet)
 {
     g_err.clear();
-    if (k < 1 || k > 32 || m < 1 || m > k || s < 1 || s > k || H < 1 || H > 32 || num_bits < 1) {
-        fail(SBF_ERR_INVALID_ARG, "sbf_create: need 1<=k<=32, 1<=m<=k, 1<=s<=k, 1<=H<=32, num_bits>=1");
+    const int sym_bits = alphabet == SBF_ALPHABET_DNA ? 2 : alphabet == SBF_ALPHABET_PROTEIN ? 5 : alphabet == SBF_ALPHABET_DNA_TRIPLET ? 6 : 0;
+    if (!sym_bits) {
+        fail(SBF_ERR_INVALID_ARG, "sbf_create_ex: unknown alphabet");
+        return nullptr;
+    }
+    if (k < 1 || k * sym_bits > 128 || m < 1 || m > k || s < 1 || s > k || H < 1 || H > 32 || num_bits < 1) {
+        fail(SBF_ERR_INVALID_ARG, "sbf_create: need 1<=k, k*symbol_bits<=128 (DNA k<=64, protein k<=25, triplets k<=21), 1<=m<=k, 1<=s<=k, 1<=H<=32, num_bits>=1");
         return nullptr;
     }
     uint64_t need = (num_bits + 255) / 256, shards = 1;
@@ -369,10 +413,12 @@ sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits)
         return nullptr;
     }
     f->k = k; f->m = m; f->s = s; f->H = H; f->P = P; f->device = dev;
+    f->alphabet = alphabet; f->sym_bits = sym_bits; f->sym_bytes = alphabet == SBF_ALPHABET_DNA_TRIPLET ? 3 : 1;
+    f->wide = alphabet != SBF_ALPHABET_DNA || k > 32;
     f->num_shards = shards;
     f->host_chunk = kHostChunkDefault;
     f->tma_flush = shards * 32 >= kTmaFlushMinBytes;
-    f->entry = P < 32 ? find_entry(k, m, s, H) : nullptr; // the specialised kernels take sigma's shift as a multiply by 2^P
+    f->entry = (P < 32 && !f->wide) ? find_entry(k, m, s, H) : nullptr; // the specialised kernels take sigma's shift as a multiply by 2^P
     e = cudaMalloc(&f->filter, shards * 32);
     if (e == cudaSuccess) e = cudaMemset(f->filter, 0, shards * 32);
     if (e == cudaSuccess) e = cudaMalloc(&f->d_flag, 256);
@@ -426,7 +472,7 @@ int sbf_reserve(sbf_t *f, uint64_t max_bases)
 int sbf_set_host_chunk(sbf_t *f, uint64_t symbols)
 {
     if (!f) return fail(SBF_ERR_INVALID_ARG, "sbf_set_host_chunk: NULL handle");
-    if (symbols == 0 || (symbols & 127) || symbols < 128 + (uint64_t)f->k)
+    if (symbols == 0 || (symbols & 127) || symbols < 128 + (uint64_t)f->k * (uint64_t)f->sym_bytes)
         return fail(SBF_ERR_INVALID_ARG, "sbf_set_host_chunk: need a multiple of 128 symbols, larger than k + 128");
     f->host_chunk = symbols;
     return SBF_OK;
@@ -599,7 +645,7 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
     }
     // the internal streams are non-blocking: order this call after everything the caller enqueued before it
     CK(cudaDeviceSynchronize());
-    const uint64_t ov = (uint64_t)f->k - 1;
+    const uint64_t ov = (uint64_t)f->k * (uint64_t)f->sym_bytes - 1; // bytes a k-mer extends past its first one
     const uint64_t kHostChunk = f->host_chunk;
     const uint64_t span = (total < kHostChunk ? total : kHostChunk) + ov; // largest chunk incl. overlap
     const uint64_t n_chunks = (total + kHostChunk - 1) / kHostChunk;
@@ -691,6 +737,7 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
             const uint64_t *lo = std::upper_bound(h_offsets + off_lo, h_offsets + n_rec + 1, a);
             const uint64_t *hi = std::lower_bound(lo, h_offsets + n_rec + 1, e);
             off_lo = (uint64_t)(lo - h_offsets);
+            f->phase0 = (int)((a - *(lo - 1)) % (uint64_t)f->sym_bytes); // triplets: the chunk's first record started at *(lo-1)
             const uint64_t n_inner = (uint64_t)(hi - lo);
             n_off = n_inner + 2;
             rebase_offsets_kernel<<<(unsigned)((n_inner + 256) / 256), 256, 0, R.comp>>>(R.d_off_full + off_lo, n_inner, a, n,
@@ -698,6 +745,7 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
             CK(cudaGetLastError());
             g_launches++;
         }
+        if (!h_offsets) f->phase0 = (int)(a % (uint64_t)f->sym_bytes);
         const char *src = h_bases + a;
         if (!direct) {
             memcpy(R.pin[sl], src, n);
@@ -713,6 +761,7 @@ int run_host(sbf *f, bool insert, const char *h_bases, const uint64_t *h_offsets
         } else {
             rc = run_query(f, R.d_bases[sl], d_off, nr, n, R.d_bitmap + a / 32, nullptr, R.comp);
         }
+        f->phase0 = 0;
         if (rc) return rc;
         CK(cudaEventRecord(R.computed[sl], R.comp));
         if (!insert && h_bitmap) {

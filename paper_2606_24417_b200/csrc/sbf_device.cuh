@@ -872,6 +872,132 @@ __global__ void __launch_bounds__(256) naive_kernel(const NaiveParams np)
 }
 
 // =============================================================================================
+// WIDE runtime-parameter kernel: the other alphabets of P:139 — protein (26 symbols, 5 bits),
+// DNA triplets (64 symbols, 6 bits, three bytes per symbol) — and packed k-mers wider than one 64-bit word (P:153,
+// P:435): k * symbol bits <= 128.  Alg. 1 / Alg. 2 as printed, one k-mer per thread, straight from the ASCII bytes
+// (no pack pass), every window recomputed.  Readings A19-A22 of DESIGN.md §3:
+//   A19 symbols; triplet symbols sit at multiples of 3 bytes from the record start, windows slide by one symbol
+//   A20 the packed k-mer is a 128-bit value, first symbol most significant
+//   A21 a window wider than 64 bits is folded before hashing: lo ^ rotl32(hi * 0x9E3779B97F4A7C15); the seeds of g and
+//       f are masked to min(window bits, 64)
+//   A22 bit index of the result bitmap = BYTE position of the k-mer's first byte
+// "Larger alphabets remain functional": this path is correct, not tuned.
+// =============================================================================================
+struct WideParams {
+    const uint8_t *bases;    // ASCII, all records concatenated
+    uint64_t total;          // bytes
+    const uint64_t *offsets; // n_rec + 1 (nullptr: one record)
+    uint64_t n_rec;
+    uint64_t *filter;
+    int shard_shift;         // 32 - P
+    uint32_t *bitmap;        // query: ceil(total/32) words, all written
+    uint64_t n_bitmap_words;
+    int k, m, s, H;
+    int alphabet;            // 0 DNA, 1 protein, 2 DNA triplet
+    int sym_bits, sym_bytes;
+    int phase0;              // bytes of the record holding byte 0 that precede the buffer, mod sym_bytes (host-facing chunks)
+};
+
+typedef unsigned __int128 u128_t;
+
+__device__ __forceinline__ int dna_code(uint32_t c)
+{
+    c &= 0xDFu;
+    return c == 'A' ? 0 : c == 'C' ? 1 : c == 'G' ? 2 : c == 'T' ? 3 : -1;
+}
+__device__ __forceinline__ int wide_symbol(const uint8_t *__restrict__ p, int alphabet)
+{
+    if (alphabet == 0) return dna_code(__ldg(p));
+    if (alphabet == 1) {
+        const uint32_t c = __ldg(p) & 0xDFu;
+        return (c >= 'A' && c <= 'Z' && (__ldg(p) & 0x40u)) ? (int)(c - 'A') : -1;
+    }
+    const int c0 = dna_code(__ldg(p)), c1 = dna_code(__ldg(p + 1)), c2 = dna_code(__ldg(p + 2));
+    return (c0 | c1 | c2) < 0 ? -1 : 16 * c0 + 4 * c1 + c2;
+}
+__device__ __forceinline__ uint64_t wide_sub(u128_t v, int k, int i, int len, int b) // Sub(v,i,len), folded (A21)
+{
+    u128_t w = v >> ((k - len - i) * b);
+    const int nb = len * b;
+    if (nb < 128) w &= (((u128_t)1) << nb) - 1;
+    const uint64_t t = (uint64_t)(w >> 64) * kGold64;
+    return (uint64_t)w ^ ((t << 32) | (t >> 32));
+}
+
+#ifdef SBF_DEFINE_AUX_KERNELS
+template <bool INSERT>
+__global__ void __launch_bounds__(256) wide_kernel(const WideParams prm)
+{
+    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; // grid covers a multiple of 32 byte positions
+    const int k = prm.k, m = prm.m, s = prm.s, H = prm.H, b = prm.sym_bits, nb = prm.sym_bytes;
+    bool present = false;
+    if (p < prm.total) {
+        // the record holding byte p: offsets[r] <= p < offsets[r+1]
+        uint64_t a = 0, e = prm.total;
+        if (prm.offsets != nullptr) {
+            uint64_t lo = 0, hi = prm.n_rec;
+            while (hi - lo > 1) {
+                const uint64_t mid = lo + (hi - lo) / 2;
+                if (__ldg(prm.offsets + mid) <= p) lo = mid; else hi = mid;
+            }
+            a = __ldg(prm.offsets + lo);
+            e = __ldg(prm.offsets + lo + 1);
+        }
+        const uint64_t rel = p - a + (a == 0 ? (uint64_t)prm.phase0 : 0);
+        if (rel % (uint64_t)nb == 0 && p + (uint64_t)k * nb <= e) {
+            u128_t v = 0;
+            bool ok = true;
+            for (int i = 0; i < k; ++i) { // ValidKmer + PackKmer (Alg. 1 l.3-4)
+                const int c = wide_symbol(prm.bases + p + (uint64_t)i * nb, prm.alphabet);
+                ok = ok && c >= 0;
+                v = (v << b) | (u128_t)(uint32_t)(c & 63);
+            }
+            if (ok) {
+                const int mb = m * b < 64 ? m * b : 64, sb = s * b < 64 ? s * b : 64;
+                uint32_t minKey = 0xFFFFFFFFu;
+                for (int i = 0; i <= k - m; ++i) { // Alg. 1 l.5-9
+                    uint64_t x = wide_sub(v, k, i, m, b) ^ (kSeedM & low_mask64(mb));
+                    minKey = min(minKey, ((uint32_t)x ^ (uint32_t)(x >> 32)) * kMultG);
+                }
+                uint64_t *sh = prm.filter + sigma_shard(minKey, prm.shard_shift) * 4;
+                uint64_t w[4] = {0, 0, 0, 0};
+                if constexpr (!INSERT) ld_shard_256(sh, w);
+                uint64_t mk[4] = {0, 0, 0, 0};
+                for (int j = 0; j <= k - s; ++j) { // Alg. 1 l.11-14 / Alg. 2 Contains
+                    uint64_t x = wide_sub(v, k, j, s, b) ^ (kSeedS & low_mask64(sb));
+                    uint64_t h = (x ^ (x >> 28)) * kMultF;
+                    h ^= h >> 32;
+                    for (int i = 0; i < H; ++i) {
+                        const uint64_t bit = 1ull << bit_pos(h, i, H);
+                        switch (i & 3) {
+                        case 0: mk[0] |= bit; break;
+                        case 1: mk[1] |= bit; break;
+                        case 2: mk[2] |= bit; break;
+                        default: mk[3] |= bit; break;
+                        }
+                    }
+                }
+                if constexpr (INSERT) {
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        if (mk[q]) red_or_64(sh + q, mk[q]);
+                } else {
+                    present = ((mk[0] & ~w[0]) | (mk[1] & ~w[1]) | (mk[2] & ~w[2]) | (mk[3] & ~w[3])) == 0;
+                }
+            }
+        }
+    }
+    if constexpr (!INSERT) {
+        const uint32_t word = __ballot_sync(0xFFFFFFFFu, present);
+        if ((threadIdx.x & 31) == 0) {
+            const uint64_t wi = p >> 5;
+            if (wi < prm.n_bitmap_words) prm.bitmap[wi] = word;
+        }
+    }
+}
+#endif // SBF_DEFINE_AUX_KERNELS
+
+// =============================================================================================
 // a6: hit counts from the result bitmap.
 // =============================================================================================
 __device__ __forceinline__ uint32_t popc_range(const uint32_t *__restrict__ bm, uint64_t a, uint64_t e)

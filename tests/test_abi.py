@@ -42,9 +42,13 @@ def test_header_has_no_torch_or_cuda_types():
 def test_invalid_arguments_fail_without_a_device():
     L = sbf.load_library()
     # bad parameters are rejected before any CUDA call
-    for args in [(0, 1, 1, 1, 1024), (33, 16, 28, 4, 1024), (31, 32, 28, 4, 1024), (31, 16, 32, 4, 1024),
+    for args in [(0, 1, 1, 1, 1024), (65, 16, 28, 4, 1024), (31, 32, 28, 4, 1024), (31, 16, 32, 4, 1024),
                  (31, 16, 28, 0, 1024), (31, 16, 28, 33, 1024), (31, 16, 28, 4, 0)]:
         assert not L.sbf_create(*args)
+        assert b"sbf_create" in L.sbf_last_error()
+    # k * symbol bits <= 128 (A20): protein k <= 25, DNA triplets k <= 21; unknown alphabet
+    for args in [(26, 6, 20, 4, 1024, sbf.ALPHABET_PROTEIN), (22, 9, 18, 4, 1024, sbf.ALPHABET_DNA_TRIPLET), (12, 6, 10, 4, 1024, 7)]:
+        assert not L.sbf_create_ex(*args)
         assert b"sbf_create" in L.sbf_last_error()
     assert L.sbf_insert_seq(None, None, 0, None) == sbf.SBF_ERR_INVALID_ARG
     assert L.sbf_query_seq(None, None, 0, None, None, None) == sbf.SBF_ERR_INVALID_ARG

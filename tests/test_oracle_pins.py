@@ -369,8 +369,13 @@ def test_p9_findere_overlap_lowers_fpr():
 
 
 def test_create_rejects_bad_parameters():
-    for args in [(0, 1, 1, 1, 256), (33, 16, 28, 4, 256), (31, 32, 28, 4, 256), (31, 16, 32, 4, 256),
+    for args in [(0, 1, 1, 1, 256), (65, 16, 28, 4, 256), (31, 32, 28, 4, 256), (31, 16, 32, 4, 256),
                  (31, 16, 28, 0, 256), (31, 16, 28, 4, 0), (31, 0, 28, 4, 256), (31, 16, 0, 4, 256)]:
+        with pytest.raises(ValueError):
+            oracle.OracleSBF(*args)
+    # the narrow (one 64-bit word) constructor still stops at k = 32; 33 <= k <= 64 is the wide path (A20)
+    assert not oracle.lib().sbfo_create(33, 16, 28, 4, 256)
+    for args in [(26, 6, 20, 4, 256, oracle.PROTEIN), (22, 9, 18, 4, 256, oracle.TRIPLET), (12, 6, 10, 4, 256, 9)]:
         with pytest.raises(ValueError):
             oracle.OracleSBF(*args)
     # A8: shard count = next power of two >= ceil(num_bits / 256)
