@@ -146,6 +146,26 @@ int sbf_query_seq_host(sbf_t *f, const char *h_seq, uint64_t len, uint32_t *h_bi
 int sbf_query_records_host(sbf_t *f, const char *h_bases, const uint64_t *h_offsets, uint64_t n_rec,
                            uint32_t *h_bitmap, uint32_t *h_hit_counts);
 
+/*
+ * FASTA / FASTQ text in HOST memory ("streamed FASTA/FASTQ input"; "Host FASTX staging").
+ *   h_text: n_bytes of uncompressed FASTA or FASTQ text (host memory; pinned memory is copied from directly).
+ *   format: 1 FASTA, 2 FASTQ, 0 = decide from the first non-blank byte ('@' -> FASTQ, anything else -> FASTA).
+ *   Text rules: lines end at '\n'; '\r' is dropped; FASTA: a line starting with '>' is a header and starts a
+ *   record, every other line is sequence of the current record (text before the first header is inserted by the
+ *   insert call and ignored by the query call); FASTQ: four lines per record (header, sequence, '+', quality;
+ *   multi-line FASTQ is not supported).  Sequence bytes are taken verbatim: validity is the alphabet's (A9 / A19).
+ * The raw text is copied to the device in chunks of sbf_set_host_chunk() bytes on one stream while the previous
+ * chunk is normalised ON THE DEVICE (headers, quality and line ends dropped, records compacted into a dense batch +
+ * offsets) and inserted / queried on another; records and k-mers may straddle chunk edges.  Synchronises.
+ *   sbf_insert_fastx_host: inserts every record.  *n_records / *n_bases (nullable) receive the number of records
+ *   (record starts) and of sequence bytes found.
+ *   sbf_query_fastx_host: h_hit_counts[r] (nullable) = number of k-mers of record r reported present, r in file
+ *   order, for r < *n_records; max_records = capacity of h_hit_counts (SBF_ERR_INVALID_ARG if the text holds more).
+ */
+int sbf_insert_fastx_host(sbf_t *f, const char *h_text, uint64_t n_bytes, int format, uint64_t *n_records, uint64_t *n_bases);
+int sbf_query_fastx_host(sbf_t *f, const char *h_text, uint64_t n_bytes, int format, uint32_t *h_hit_counts,
+                         uint64_t max_records, uint64_t *n_records, uint64_t *n_bases);
+
 /* sbf_set_host_chunk — symbols per staged chunk of the host-facing calls ("multi-chunk workloads"):
  * a multiple of 128, larger than k + 128; default 32 Mi (the measured optimum on B200 / PCIe 5).  Chunks overlap by
  * k-1 symbols so that every k-mer lies wholly inside one chunk.  A tuning knob; tests use small chunks to put

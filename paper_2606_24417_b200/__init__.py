@@ -45,6 +45,8 @@ ABI = {
     "sbf_insert_records_host": (_i32, [_p, _p, _p, _u64]),
     "sbf_query_seq_host": (_i32, [_p, _p, _u64, _p, _p]),
     "sbf_query_records_host": (_i32, [_p, _p, _p, _u64, _p, _p]),
+    "sbf_insert_fastx_host": (_i32, [_p, _p, _u64, _i32, _p, _p]),
+    "sbf_query_fastx_host": (_i32, [_p, _p, _u64, _i32, _p, _u64, _p, _p]),
     "sbf_export_bits": (_i32, [_p, _p, _u64]),
     "sbf_import_bits": (_i32, [_p, _p, _u64]),
     "sbf_filter_device_ptr": (_p, [_p]),
@@ -118,6 +120,8 @@ def _hptr(x) -> Optional[int]:
         return None
     if isinstance(x, int):
         return x
+    if isinstance(x, bytes):   # the caller keeps the object alive for the duration of the call
+        return ctypes.cast(ctypes.c_char_p(x), ctypes.c_void_p).value
     if isinstance(x, np.ndarray):
         if not x.flags["C_CONTIGUOUS"]:
             raise TypeError("expected a C-contiguous array")
@@ -199,6 +203,21 @@ def sbf_query_seq_host(h, h_seq, length: int, h_bitmap, h_hits=None):
 def sbf_query_records_host(h, h_bases, h_offsets, n_rec: int, h_bitmap, h_hit_counts=None):
     _check(load_library().sbf_query_records_host(h, _hptr(h_bases), _hptr(h_offsets), n_rec, _hptr(h_bitmap),
                                                  _hptr(h_hit_counts)))
+
+
+def sbf_insert_fastx_host(h, h_text, n_bytes: int, fmt: int = 0):
+    """(records, sequence bytes) found in the FASTA/FASTQ text and inserted."""
+    nr, nb = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    _check(load_library().sbf_insert_fastx_host(h, _hptr(h_text), n_bytes, fmt, ctypes.addressof(nr), ctypes.addressof(nb)))
+    return int(nr.value), int(nb.value)
+
+
+def sbf_query_fastx_host(h, h_text, n_bytes: int, h_hit_counts, max_records: int, fmt: int = 0):
+    """Fills h_hit_counts[0 .. records); returns (records, sequence bytes)."""
+    nr, nb = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    _check(load_library().sbf_query_fastx_host(h, _hptr(h_text), n_bytes, fmt, _hptr(h_hit_counts), max_records,
+                                               ctypes.addressof(nr), ctypes.addressof(nb)))
+    return int(nr.value), int(nb.value)
 
 
 def sbf_export_bits(h) -> np.ndarray:

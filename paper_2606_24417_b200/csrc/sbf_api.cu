@@ -13,6 +13,7 @@
 
 #define SBF_DEFINE_AUX_KERNELS
 #include "sbf_dispatch.h"
+#include "sbf_fastx.cuh"
 
 using namespace sbfk;
 
@@ -98,6 +99,40 @@ struct HostRun { // persistent state of the host-facing path (two slots: copy c+
     }
 };
 
+struct FastxRun { // persistent state of the FASTX host path (two slots: copy chunk c+1 while chunk c is normalised and walked)
+    cudaStream_t copy = nullptr, comp = nullptr;
+    cudaEvent_t copied[2] = {nullptr, nullptr}, computed[2] = {nullptr, nullptr}, normalised = nullptr;
+    char *pin[2] = {nullptr, nullptr};
+    uint8_t *d_text[2] = {nullptr, nullptr}, *d_dense[2] = {nullptr, nullptr};
+    uint64_t *d_off[2] = {nullptr, nullptr};
+    uint64_t cap_text = 0; // bytes of text per slot the buffers above are sized for
+    Seg *d_tiles = nullptr;
+    FastxState *d_state = nullptr, *h_state = nullptr; // 2 device states (alternating), one pinned host copy
+    uint32_t *d_bitmap = nullptr, *d_counts_local = nullptr, *d_counts = nullptr;
+    uint64_t cap_counts = 0;
+    ~FastxRun()
+    {
+        for (int i = 0; i < 2; ++i) {
+            if (copied[i]) cudaEventDestroy(copied[i]);
+            if (computed[i]) cudaEventDestroy(computed[i]);
+            if (pin[i]) cudaFreeHost(pin[i]);
+            if (d_text[i]) cudaFree(d_text[i]);
+            if (d_dense[i]) cudaFree(d_dense[i]);
+            if (d_off[i]) cudaFree(d_off[i]);
+        }
+        if (normalised) cudaEventDestroy(normalised);
+        if (d_tiles) cudaFree(d_tiles);
+        if (d_state) cudaFree(d_state);
+        if (h_state) cudaFreeHost(h_state);
+        if (d_bitmap) cudaFree(d_bitmap);
+        if (d_counts_local) cudaFree(d_counts_local);
+        if (d_counts) cudaFree(d_counts);
+        if (copy) cudaStreamDestroy(copy);
+        if (comp) cudaStreamDestroy(comp);
+        cudaGetLastError();
+    }
+};
+
 } // namespace
 
 namespace sbfk {
@@ -135,6 +170,7 @@ struct sbf {
     bool l2_stream_valid;
     // host-facing staging (created on first use)
     HostRun *host;
+    FastxRun *fastx;          // FASTX host path (created on first use)
     uint64_t host_chunk;      // symbols per staged chunk (sbf_set_host_chunk; default kHostChunkDefault)
     // optional per-kernel timing (sbf_set_timing): events on the caller's stream around each kernel
     bool timing;
@@ -448,6 +484,7 @@ void sbf_destroy(sbf_t *f)
     if (!f) return;
     cudaDeviceSynchronize();
     delete f->host;
+    delete f->fastx;
     for (int i = 0; i < 4; ++i)
         if (f->tev[i]) cudaEventDestroy(f->tev[i]);
     if (f->packed) cudaFree(f->packed);
@@ -822,6 +859,202 @@ int sbf_query_records_host(sbf_t *f, const char *h_bases, const uint64_t *h_offs
     uint64_t total = h_offsets[n_rec];
     if ((!h_bases || !h_bitmap) && total) return fail(SBF_ERR_INVALID_ARG, "sbf_query_records_host: NULL buffer");
     return run_host(f, false, h_bases, h_offsets, n_rec, total, h_bitmap, h_hit_counts, nullptr);
+}
+
+} // extern "C"
+
+// =============================================================================================
+// C ABI — FASTA / FASTQ text in host memory ("streamed FASTA/FASTQ input"; "Host FASTX staging").
+// The raw text is cut in chunks of host_chunk bytes; a copy stream moves chunk c+1 to the device while the compute
+// stream normalises chunk c there (sbf_fastx.cuh: headers, quality lines and line ends dropped, sequence bytes
+// compacted into a dense record batch + offsets) and runs the ordinary record-batch insert / query on it.  The lexer
+// state and the last k-1 bytes of the open record travel from chunk to chunk in device memory; the host reads back
+// 24 bytes per chunk (the batch's size), which is what it needs to size the launches.
+// =============================================================================================
+namespace {
+
+template <int FMT>
+int fastx_normalise_chunk(FastxRun &R, int sl, uint64_t n, const FastxState *st, FastxState *st_next, uint32_t keep, bool last)
+{
+    const uint32_t n_tiles = (uint32_t)((n + kFxTile - 1) / kFxTile);
+    if (n_tiles) {
+        fastx_tile_kernel<FMT><<<n_tiles, kFxThreads, 0, R.comp>>>(R.d_text[sl], n, st, R.d_tiles);
+        CK(cudaGetLastError());
+    }
+    fastx_scan_kernel<FMT><<<1, 32, 0, R.comp>>>(R.d_tiles, n_tiles, R.d_text[sl], n, const_cast<FastxState *>(st), st_next, R.d_off[sl]);
+    CK(cudaGetLastError());
+    if (n_tiles) {
+        fastx_emit_kernel<FMT><<<n_tiles, kFxThreads, 0, R.comp>>>(R.d_text[sl], n, st, R.d_tiles, R.d_dense[sl], R.d_off[sl]);
+        CK(cudaGetLastError());
+    }
+    g_launches += n_tiles ? 3 : 1;
+    if (!last) {
+        fastx_carry_kernel<<<1, 64, 0, R.comp>>>(R.d_dense[sl], R.d_off[sl], st, keep, R.d_dense[sl ^ 1], st_next);
+        CK(cudaGetLastError());
+        g_launches++;
+    }
+    return SBF_OK;
+}
+
+int run_fastx(sbf *f, bool insert, const char *h_text, uint64_t n_bytes, int format, uint32_t *h_counts, uint64_t max_records,
+              uint64_t *out_records, uint64_t *out_bases)
+{
+    if (out_records) *out_records = 0;
+    if (out_bases) *out_bases = 0;
+    if (format == 0) { // detect from the first byte that is not white space
+        uint64_t i = 0;
+        while (i < n_bytes && (h_text[i] == '\n' || h_text[i] == '\r' || h_text[i] == ' ')) ++i;
+        format = (i < n_bytes && h_text[i] == '@') ? kFxFastq : kFxFasta;
+    }
+    if (format != kFxFasta && format != kFxFastq) return fail(SBF_ERR_INVALID_ARG, "fastx: format must be 0 (detect), 1 (FASTA) or 2 (FASTQ)");
+    if (n_bytes == 0) return SBF_OK;
+    CK(cudaDeviceSynchronize()); // order this call after everything enqueued before it (the internal streams are non-blocking)
+    const uint64_t chunk = f->host_chunk;
+    const uint64_t n_chunks = (n_bytes + chunk - 1) / chunk;
+    const uint32_t keep = (uint32_t)(f->k * f->sym_bytes - 1);
+    const uint64_t span = (n_bytes < chunk ? n_bytes : chunk);
+    if (!f->fastx) {
+        f->fastx = new (std::nothrow) FastxRun();
+        if (!f->fastx) return fail(SBF_ERR_NOMEM, "fastx: allocation failed");
+        FastxRun &N = *f->fastx;
+        CK(cudaStreamCreateWithFlags(&N.copy, cudaStreamNonBlocking));
+        CK(cudaStreamCreateWithFlags(&N.comp, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CK(cudaEventCreateWithFlags(&N.copied[i], cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&N.computed[i], cudaEventDisableTiming));
+        }
+        CK(cudaEventCreateWithFlags(&N.normalised, cudaEventDisableTiming));
+        CK(cudaMalloc(&N.d_state, 2 * sizeof(FastxState)));
+        CK(cudaMallocHost(&N.h_state, sizeof(FastxState)));
+    }
+    FastxRun &R = *f->fastx;
+    const bool direct = is_pinned(h_text);
+    if (R.cap_text < span) { // every buffer below is sized by the text bytes of one chunk
+        for (int i = 0; i < 2; ++i) {
+            if (R.pin[i]) cudaFreeHost(R.pin[i]);
+            if (R.d_text[i]) cudaFree(R.d_text[i]);
+            if (R.d_dense[i]) cudaFree(R.d_dense[i]);
+            if (R.d_off[i]) cudaFree(R.d_off[i]);
+            R.pin[i] = nullptr; R.d_text[i] = nullptr; R.d_dense[i] = nullptr; R.d_off[i] = nullptr;
+        }
+        if (R.d_tiles) cudaFree(R.d_tiles);
+        if (R.d_bitmap) cudaFree(R.d_bitmap);
+        if (R.d_counts_local) cudaFree(R.d_counts_local);
+        R.d_tiles = nullptr; R.d_bitmap = nullptr; R.d_counts_local = nullptr; R.cap_text = 0;
+        const uint64_t max_rec = span / 2 + 3; // a record start needs ">" and a line end before the next one
+        for (int i = 0; i < 2; ++i) {
+            CK(cudaMallocHost(&R.pin[i], span));
+            CK(cudaMalloc(&R.d_text[i], span + 16));
+            CK(cudaMalloc(&R.d_dense[i], span + keep + 64));
+            CK(cudaMalloc(&R.d_off[i], (max_rec + 2) * sizeof(uint64_t)));
+        }
+        CK(cudaMalloc(&R.d_tiles, ((span + kFxTile - 1) / kFxTile + 1) * sizeof(Seg)));
+        CK(cudaMalloc(&R.d_bitmap, ((span + keep + 64 + 31) / 32 + 4) * sizeof(uint32_t)));
+        CK(cudaMalloc(&R.d_counts_local, (max_rec + 2) * sizeof(uint32_t)));
+        R.cap_text = span;
+    }
+    if (!insert && h_counts && max_records) {
+        if (R.cap_counts < max_records) {
+            if (R.d_counts) cudaFree(R.d_counts);
+            R.d_counts = nullptr; R.cap_counts = 0;
+            CK(cudaMalloc(&R.d_counts, max_records * sizeof(uint32_t)));
+            R.cap_counts = max_records;
+        }
+        CK(cudaMemsetAsync(R.d_counts, 0, max_records * sizeof(uint32_t), R.comp));
+    }
+    int rc = ensure_scratch(f, span + keep + 64);
+    if (rc) return rc;
+    FastxState init;
+    memset(&init, 0, sizeof(init));
+    init.at_line_start = 1;
+    CK(cudaMemcpyAsync(&R.d_state[0], &init, sizeof(init), cudaMemcpyHostToDevice, R.comp));
+
+    uint64_t rec_base = 0, bases_total = 0; // record starts / distinct sequence bytes before the current chunk
+    uint32_t rec_prefix = 0;                // triplets: bytes of local record 0 that precede the dense buffer, mod 3
+    for (uint64_t c = 0; c < n_chunks; ++c) {
+        const int sl = (int)(c & 1);
+        const uint64_t a = c * chunk;
+        const uint64_t n = (a + chunk < n_bytes) ? chunk : n_bytes - a;
+        if (c >= 2) {
+            CK(cudaEventSynchronize(R.copied[sl]));
+            CK(cudaStreamWaitEvent(R.copy, R.computed[sl], 0));
+        }
+        const char *src = h_text + a;
+        if (!direct) {
+            memcpy(R.pin[sl], src, n);
+            src = R.pin[sl];
+        }
+        CK(cudaMemcpyAsync(R.d_text[sl], src, n, cudaMemcpyHostToDevice, R.copy));
+        CK(cudaEventRecord(R.copied[sl], R.copy));
+        CK(cudaStreamWaitEvent(R.comp, R.copied[sl], 0));
+        FastxState *st = &R.d_state[c & 1], *st_next = &R.d_state[(c + 1) & 1];
+        const bool last = c + 1 == n_chunks;
+        rc = format == kFxFasta ? fastx_normalise_chunk<kFxFasta>(R, sl, n, st, st_next, keep, last)
+                                : fastx_normalise_chunk<kFxFastq>(R, sl, n, st, st_next, keep, last);
+        if (rc) return rc;
+        CK(cudaMemcpyAsync(R.h_state, st, sizeof(FastxState), cudaMemcpyDeviceToHost, R.comp));
+        CK(cudaEventRecord(R.normalised, R.comp));
+        CK(cudaEventSynchronize(R.normalised)); // 40 bytes: the batch's size, needed to size the launches below
+        const uint64_t n_bases = R.h_state->n_bases, n_starts = R.h_state->n_starts, carry = R.h_state->carry_len;
+        const uint64_t n_rec = n_starts + 1;
+        if (!insert && h_counts && rec_base + n_starts > max_records)
+            return fail(SBF_ERR_INVALID_ARG, "sbf_query_fastx_host: more records in the text than max_records");
+        f->phase0 = (int)(rec_prefix % (uint32_t)f->sym_bytes);
+        if (n_bases) {
+            if (insert) {
+                rc = run_insert(f, reinterpret_cast<const char *>(R.d_dense[sl]), R.d_off[sl], n_rec, n_bases, R.comp);
+            } else {
+                rc = run_query(f, reinterpret_cast<const char *>(R.d_dense[sl]), R.d_off[sl], n_rec, n_bases, R.d_bitmap,
+                               h_counts ? R.d_counts_local : nullptr, R.comp);
+                if (!rc && h_counts) {
+                    unsigned blocks = (unsigned)((n_rec + 255) / 256 < 1184 ? (n_rec + 255) / 256 : 1184);
+                    fastx_add_counts_kernel<<<blocks, 256, 0, R.comp>>>(R.d_counts_local, n_rec, rec_base, R.d_counts, max_records);
+                    rc = cudaGetLastError() == cudaSuccess ? SBF_OK : fail(SBF_ERR_CUDA, "fastx_add_counts_kernel");
+                    g_launches++;
+                }
+            }
+        }
+        f->phase0 = 0;
+        if (rc) return rc;
+        CK(cudaEventRecord(R.computed[sl], R.comp));
+        // the record that is open at the end of this chunk: how many of its bytes the next dense buffer will NOT hold
+        // (host mirror of fastx_carry_kernel's choice; needs the last record's length, which the offsets hold on the
+        // device — read back only for multi-byte symbols, where the 3-byte grid must survive the chunk edge)
+        if (!last && f->sym_bytes > 1) {
+            uint64_t last_start = 0;
+            CK(cudaMemcpyAsync(&last_start, R.d_off[sl] + n_starts, sizeof(uint64_t), cudaMemcpyDeviceToHost, R.comp));
+            CK(cudaStreamSynchronize(R.comp));
+            const uint64_t len = n_bases - last_start;
+            const uint64_t cl = len < keep ? len : keep;
+            rec_prefix = (uint32_t)(((n_starts ? 0 : rec_prefix) + len - cl) % 3);
+        }
+        rec_base += n_starts;
+        bases_total += n_bases - carry;
+    }
+    if (!insert && h_counts && rec_base)
+        CK(cudaMemcpyAsync(h_counts, R.d_counts, rec_base * sizeof(uint32_t), cudaMemcpyDeviceToHost, R.comp));
+    CK(cudaStreamSynchronize(R.copy));
+    CK(cudaStreamSynchronize(R.comp));
+    if (out_records) *out_records = rec_base;
+    if (out_bases) *out_bases = bases_total;
+    return SBF_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int sbf_insert_fastx_host(sbf_t *f, const char *h_text, uint64_t n_bytes, int format, uint64_t *n_records, uint64_t *n_bases)
+{
+    if (!f || (!h_text && n_bytes)) return fail(SBF_ERR_INVALID_ARG, "sbf_insert_fastx_host: NULL argument");
+    return run_fastx(f, true, h_text, n_bytes, format, nullptr, 0, n_records, n_bases);
+}
+
+int sbf_query_fastx_host(sbf_t *f, const char *h_text, uint64_t n_bytes, int format, uint32_t *h_hit_counts, uint64_t max_records,
+                         uint64_t *n_records, uint64_t *n_bases)
+{
+    if (!f || (!h_text && n_bytes)) return fail(SBF_ERR_INVALID_ARG, "sbf_query_fastx_host: NULL argument");
+    return run_fastx(f, false, h_text, n_bytes, format, h_hit_counts, h_hit_counts ? max_records : 0, n_records, n_bases);
 }
 
 } // extern "C"

@@ -155,6 +155,32 @@ def uniform_device(seed: int, first: int, n: int, out=None, stream=None):
     return out
 
 
+def fasta_text(records, width: int = 60, crlf: bool = False, names=None) -> bytes:
+    """FASTA text of the given records (uint8 arrays / bytes): '>name' line, then the sequence wrapped at `width`."""
+    eol = b"\r\n" if crlf else b"\n"
+    out = bytearray()
+    for i, r in enumerate(records):
+        b = bytes(r)
+        out += b">" + (names[i] if names else b"rec%d some description" % i) + eol
+        for a in range(0, len(b), width):
+            out += b[a:a + width] + eol
+    return bytes(out)
+
+
+def fastq_text(records, crlf: bool = False, final_newline: bool = True) -> bytes:
+    """Four-line FASTQ text of the given records; the quality line is a seeded pattern that contains '>' and '@'."""
+    eol = b"\r\n" if crlf else b"\n"
+    qual = b"IIII>@FF#5;"
+    out = bytearray()
+    for i, r in enumerate(records):
+        b = bytes(r)
+        q = (qual * (len(b) // len(qual) + 1))[:len(b)]
+        out += b"@read%d/1" % i + eol + b + eol + b"+" + eol + q + eol
+    if not final_newline and out.endswith(eol):
+        del out[-len(eol):]
+    return bytes(out)
+
+
 def fixed_offsets(n_reads: int, read_len: int, first: int = 0) -> np.ndarray:
     """offsets[n_reads+1] of back-to-back fixed-length records (relative to the batch)."""
     return (np.arange(n_reads + 1, dtype=np.uint64) * np.uint64(read_len))
