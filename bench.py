@@ -470,13 +470,15 @@ def run_cuda(args):
         rs = ceilings["random_sector_g_per_s"]
         ins_runs_g = n_ins_kmers * d_runs / (ik * 1e-3) / 1e9
         q_runs_g = qk_kmers * (d_runs + 1.0 / per_read) / (qk * 1e-3) / 1e9
-        rmw_ceiling = max(x for x in (rs.get("red_or_b64_x4"), rs.get("red_or_b64_x1")) if x)  # the better of the two
+        # the best any read-modify-write form reached (1 RED, 4 REDs, one 32-byte TMA reduction) / any load form
+        rmw_ceiling = max(x for x in (rs.get("red_or_b64_x4"), rs.get("red_or_b64_x1"), rs.get("tma_reduce_or_32B")) if x)
+        ld_ceiling = max(x for x in (rs.get("ld_nc_256"), rs.get("cp_async_2x16")) if x)
         roof["insert_kernel"]["random_sector"] = {
             "achieved_g_per_s": ins_runs_g, "ceiling_g_per_s": rmw_ceiling, "frac": ins_runs_g / rmw_ceiling,
-            "ceiling": "random red.or.b64 sectors/s over %d MiB, best of 1 and 4 RED per sector" % (num_bits >> 23)}
+            "ceiling": "random read-modify-write sectors/s over %d MiB, best of 1 RED, 4 REDs, one TMA reduction" % (num_bits >> 23)}
         roof["query_kernel"]["random_sector"] = {
-            "achieved_g_per_s": q_runs_g, "ceiling_g_per_s": rs["cp_async_2x16"], "frac": q_runs_g / rs["cp_async_2x16"],
-            "ceiling": "random 2 x 16-byte cp.async sectors/s over %d MiB" % (num_bits >> 23)}
+            "achieved_g_per_s": q_runs_g, "ceiling_g_per_s": ld_ceiling, "frac": q_runs_g / ld_ceiling,
+            "ceiling": "random sector loads/s over %d MiB, best of one 256-bit ld.global.nc and 2 x 16-byte cp.async" % (num_bits >> 23)}
         for kk in ("insert_kernel", "query_kernel"):  # which limit binds this kernel: instructions or random sectors
             r = roof[kk]
             busy = dict(r.get("busy_fraction_of_measured_limit", {"alu_pipe": r["frac"]}))

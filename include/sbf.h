@@ -189,6 +189,20 @@ int sbf_or_bits_device(sbf_t *f, const uint64_t *d_src, uint64_t nbytes, void *s
  * replica merge run window by window (paper_2606_24417_b200/replicas.py). */
 int sbf_or_range_device(sbf_t *f, uint64_t offset_bytes, const uint64_t *d_src, uint64_t nbytes, void *stream);
 
+/* sbf_or_peers_range_device — filter[offset_bytes .. +nbytes) |= OR over n_peers (<= 15) replicas of the SAME range,
+ * each given by a device pointer to the start of its range and read in place: peer-GPU memory mapped through CUDA IPC
+ * (sbf_ipc_open_filter) over NVLink, or other filters on this device.  The reduce-scatter step of the replica merge as
+ * one kernel per window, without a receive buffer (paper_2606_24417_b200/replicas.py: or_allreduce_filter_peer).
+ * d_peer_ranges is a HOST array of device pointers (16-byte aligned); stream-ordered. */
+int sbf_or_peers_range_device(sbf_t *f, uint64_t offset_bytes, const uint64_t *const *d_peer_ranges, int n_peers, uint64_t nbytes,
+                              void *stream);
+/* CUDA IPC plumbing for the above: export this filter's allocation as a 64-byte handle another process (rank) of the
+ * same node can open; open / close a peer's.  The mapping gives direct loads over NVLink (peer access is enabled
+ * lazily).  Never executed on more than one GPU in this repository's test environment (one GPU per box). */
+int sbf_ipc_export_filter(const sbf_t *f, void *handle64);
+int sbf_ipc_open_filter(const void *handle64, uint64_t **d_ptr);
+int sbf_ipc_close_filter(uint64_t *d_ptr);
+
 /* Message for the last error on the calling thread ("" if none). */
 const char *sbf_last_error(void);
 

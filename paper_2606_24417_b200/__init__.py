@@ -52,6 +52,10 @@ ABI = {
     "sbf_filter_device_ptr": (_p, [_p]),
     "sbf_or_bits_device": (_i32, [_p, _p, _u64, _p]),
     "sbf_or_range_device": (_i32, [_p, _u64, _p, _u64, _p]),
+    "sbf_or_peers_range_device": (_i32, [_p, _u64, _p, _i32, _u64, _p]),
+    "sbf_ipc_export_filter": (_i32, [_p, _p]),
+    "sbf_ipc_open_filter": (_i32, [_p, _p]),
+    "sbf_ipc_close_filter": (_i32, [_p]),
     "sbf_last_error": (_cp, []),
     "sbf_kernel_launches": (_u64, []),
     "sbf_set_host_chunk": (_i32, [_p, _u64]),
@@ -239,6 +243,30 @@ def sbf_or_bits_device(h, d_src, nbytes: int, stream=None):
 
 def sbf_or_range_device(h, offset_bytes: int, d_src, nbytes: int, stream=None):
     _check(load_library().sbf_or_range_device(h, offset_bytes, _dptr(d_src), nbytes, _stream(stream)))
+
+
+def sbf_or_peers_range_device(h, offset_bytes: int, peer_range_ptrs, nbytes: int, stream=None):
+    """peer_range_ptrs: raw device pointers (ints) to the start of the same range in every peer replica."""
+    arr = (ctypes.c_uint64 * max(1, len(peer_range_ptrs)))(*peer_range_ptrs)
+    _check(load_library().sbf_or_peers_range_device(h, offset_bytes, ctypes.addressof(arr), len(peer_range_ptrs), nbytes,
+                                                    _stream(stream)))
+
+
+def sbf_ipc_export_filter(h) -> bytes:
+    buf = ctypes.create_string_buffer(64)
+    _check(load_library().sbf_ipc_export_filter(h, ctypes.addressof(buf)))
+    return buf.raw
+
+
+def sbf_ipc_open_filter(handle64: bytes) -> int:
+    buf = ctypes.create_string_buffer(handle64, 64)
+    out = ctypes.c_uint64(0)
+    _check(load_library().sbf_ipc_open_filter(ctypes.addressof(buf), ctypes.addressof(out)))
+    return int(out.value)
+
+
+def sbf_ipc_close_filter(ptr: int):
+    _check(load_library().sbf_ipc_close_filter(ptr))
 
 
 def sbf_set_host_chunk(h, symbols: int):

@@ -638,6 +638,55 @@ int sbf_or_range_device(sbf_t *f, uint64_t offset_bytes, const uint64_t *d_src, 
     return SBF_OK;
 }
 
+int sbf_or_peers_range_device(sbf_t *f, uint64_t offset_bytes, const uint64_t *const *d_peer_ranges, int n_peers, uint64_t nbytes,
+                              void *stream)
+{
+    if (!f || (!d_peer_ranges && n_peers)) return fail(SBF_ERR_INVALID_ARG, "sbf_or_peers_range_device: NULL argument");
+    if (n_peers < 0 || n_peers > kMaxPeers) return fail(SBF_ERR_INVALID_ARG, "sbf_or_peers_range_device: at most 15 peers per call");
+    if ((offset_bytes & 31) || (nbytes & 31) || offset_bytes + nbytes > f->num_shards * 32)
+        return fail(SBF_ERR_INVALID_ARG, "sbf_or_peers_range_device: range must be whole shards inside the filter");
+    PeerPtrs pp;
+    for (int j = 0; j < kMaxPeers; ++j) pp.p[j] = nullptr;
+    for (int j = 0; j < n_peers; ++j) {
+        if (!d_peer_ranges[j] || (reinterpret_cast<uintptr_t>(d_peer_ranges[j]) & 15))
+            return fail(SBF_ERR_INVALID_ARG, "sbf_or_peers_range_device: peer pointers must be non-NULL and 16-byte aligned");
+        pp.p[j] = d_peer_ranges[j];
+    }
+    const uint64_t nw = nbytes / 8;
+    if (nw == 0 || n_peers == 0) return SBF_OK;
+    unsigned blocks = (unsigned)((nw / 2 + 255) / 256 < 2368 ? (nw / 2 + 255) / 256 : 2368);
+    or_peers_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(f->filter + offset_bytes / 8, pp, n_peers, nw);
+    CK(cudaGetLastError());
+    g_launches++;
+    return SBF_OK;
+}
+
+int sbf_ipc_export_filter(const sbf_t *f, void *handle64)
+{
+    if (!f || !handle64) return fail(SBF_ERR_INVALID_ARG, "sbf_ipc_export_filter: NULL argument");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "cudaIpcMemHandle_t is 64 bytes");
+    CK(cudaIpcGetMemHandle(reinterpret_cast<cudaIpcMemHandle_t *>(handle64), f->filter));
+    return SBF_OK;
+}
+
+int sbf_ipc_open_filter(const void *handle64, uint64_t **d_ptr)
+{
+    if (!handle64 || !d_ptr) return fail(SBF_ERR_INVALID_ARG, "sbf_ipc_open_filter: NULL argument");
+    cudaIpcMemHandle_t h;
+    memcpy(&h, handle64, sizeof(h));
+    void *p = nullptr;
+    CK(cudaIpcOpenMemHandle(&p, h, cudaIpcMemLazyEnablePeerAccess));
+    *d_ptr = static_cast<uint64_t *>(p);
+    return SBF_OK;
+}
+
+int sbf_ipc_close_filter(uint64_t *d_ptr)
+{
+    if (!d_ptr) return SBF_OK;
+    CK(cudaIpcCloseMemHandle(d_ptr));
+    return SBF_OK;
+}
+
 int sbf_debug_last_packed(const sbf_t *f, uint32_t *h_words, uint16_t *h_mask, uint64_t n_words)
 {
     if (!f || !h_words || !h_mask) return fail(SBF_ERR_INVALID_ARG, "sbf_debug_last_packed: NULL argument");

@@ -248,12 +248,14 @@ __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ s
     // V = OR of k consecutive B bits, by doubling: after the loop bit j of y covers B[j .. j+c-1], c the largest power
     // of two <= k; one more step with the remainder closes the window (k - c <= c)
     uint64_t y = (uint64_t)inv | ((uint64_t)nxt << 32);
-    int c = 1;
-    while (2 * c <= k) {
-        y |= y >> c;
-        c *= 2;
+    if (__any_sync(0xFFFFFFFFu, y != 0)) { // almost every warp sees only valid symbols: V = 0 without the doubling
+        int c = 1;
+        while (2 * c <= k) {
+            y |= y >> c;
+            c *= 2;
+        }
+        if (c < k) y |= y >> (k - c);
     }
-    if (c < k) y |= y >> (k - c);
     const uint32_t g = (uint32_t)y;
     if (2 * i + 1 < n_words_total) {
         *reinterpret_cast<uint2 *>(packed + 2 * i) = make_uint2(word[0], word[1]);
@@ -1084,6 +1086,25 @@ __global__ void __launch_bounds__(256) or_words_kernel(uint64_t *__restrict__ ds
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (uint64_t)gridDim.x * blockDim.x) {
         ulonglong2 a = d2[i], b = s2[i];
         a.x |= b.x; a.y |= b.y;
+        d2[i] = a;
+    }
+}
+
+// filter[range] |= OR over the peers' replicas of the same range, read in place through peer pointers (NVLink P2P / CUDA
+// IPC mappings, or other filters on this device): the reduce-scatter step of the replica merge as ONE kernel per
+// window — no staging buffer, no separate receive.  src holds up to kMaxPeers device pointers to the START of the range.
+constexpr int kMaxPeers = 15;
+struct PeerPtrs { const uint64_t *p[kMaxPeers]; };
+__global__ void __launch_bounds__(256) or_peers_kernel(uint64_t *__restrict__ dst, PeerPtrs src, int n_src, uint64_t n_words)
+{
+    const uint64_t n2 = n_words / 2;
+    ulonglong2 *d2 = reinterpret_cast<ulonglong2 *>(dst);
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += (uint64_t)gridDim.x * blockDim.x) {
+        ulonglong2 a = d2[i];
+        for (int j = 0; j < n_src; ++j) {
+            const ulonglong2 b = reinterpret_cast<const ulonglong2 *>(src.p[j])[i];
+            a.x |= b.x; a.y |= b.y;
+        }
         d2[i] = a;
     }
 }

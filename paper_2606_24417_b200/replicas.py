@@ -171,3 +171,94 @@ def or_allreduce_filter(handle, group=None, stream=None, window_bytes: int = 1 <
 
     with torch.cuda.stream(st):
         return or_allreduce(filter_tensor(handle), or_into, group=group, window_bytes=window_bytes)
+
+
+# ---- peer-memory form of the exchange: each rank ORs its slice straight out of its peers' filters ---------------
+def merge_plan(n_bytes: int, world: int, window_bytes: int = 1 << 28):
+    """The windows and per-rank slices the exchange walks: [(window_offset, [(slice_lo, slice_hi) per rank])], all in
+    bytes, slices relative to the window and cut on shard (32-byte) boundaries.  Pure arithmetic (tested on CPU)."""
+    assert n_bytes % 32 == 0
+    window = min(n_bytes, max(32 * world, window_bytes - window_bytes % 32))
+    return [(a, _slices(min(window, n_bytes - a), world)) for a in range(0, n_bytes, window)]
+
+
+def merge_local_replicas(handles, window_bytes: int = 1 << 28, stream=None) -> int:
+    """Replicas that live on ONE device (e.g. filled on different streams): afterwards every one holds the OR of all.
+    Walks the same plan as the multi-GPU exchange with the same kernels — `sbf_or_peers_range_device` reads the
+    other replicas in place for the reduce-scatter step, the reduced slices are then copied back out — so a single
+    GPU exercises the window / slice arithmetic and the peer-read kernel of `or_allreduce_filter_peer`.
+    Returns the number of peer-read kernel launches."""
+    import torch
+    from . import sbf_filter_device_ptr, sbf_num_shards, sbf_or_peers_range_device
+
+    world = len(handles)
+    n = sbf_num_shards(handles[0]) * 32
+    assert all(sbf_num_shards(h) * 32 == n for h in handles)
+    base = [sbf_filter_device_ptr(h) for h in handles]
+    tens = [filter_tensor(h) for h in handles]
+    launches = 0
+    ctx = torch.cuda.stream(stream) if stream is not None else _null_ctx()
+    with ctx:
+        for a, slices in merge_plan(n, world, window_bytes):
+            for j, (lo, hi) in enumerate(slices):          # "rank" j reduces its slice of this window
+                if hi > lo:
+                    peers = [base[p] + a + lo for p in range(world) if p != j]
+                    sbf_or_peers_range_device(handles[j], a + lo, peers, hi - lo, stream)
+                    launches += 1
+            for j, (lo, hi) in enumerate(slices):          # all-gather: every replica takes slice j from its owner
+                for p in range(world):
+                    if p != j and hi > lo:
+                        tens[p][a + lo:a + hi].copy_(tens[j][a + lo:a + hi], non_blocking=True)
+    return launches
+
+
+class _null_ctx:
+    def __enter__(self): return self
+    def __exit__(self, *a): return False
+
+
+def or_allreduce_filter_peer(handle, group=None, stream=None, window_bytes: int = 1 << 28) -> int:
+    """The exchange over NVLink peer memory ("a peer-read reduce-scatter/all-gather kernel"): every
+    rank maps its peers' filters through CUDA IPC once, then per window (1) ORs its own slice straight out of the
+    peers' filters with ONE kernel (`sbf_or_peers_range_device`: N-1 remote reads per word, no receive buffer, no
+    separate OR pass), (2) after a barrier copies the other ranks' finished slices out of their filters.  2 (N-1)/N
+    filters cross NVLink per rank, as in the NCCL form, but without staging and with the reduce fused into the transfer.
+    Ranks must share a node (CUDA IPC).  NEVER RUN ON MORE THAN ONE GPU in this repository's environment (one GPU per
+    box): the plan and the kernel are exercised by `merge_local_replicas` on one device, the IPC mapping is not."""
+    import torch
+    import torch.distributed as dist
+    from . import (sbf_filter_device_ptr, sbf_ipc_close_filter, sbf_ipc_export_filter, sbf_ipc_open_filter, sbf_num_shards,
+                   sbf_or_peers_range_device)
+
+    world, rank = dist.get_world_size(group), dist.get_rank(group)
+    if world == 1:
+        return 0
+    st = torch.cuda.current_stream() if stream is None else (torch.cuda.ExternalStream(stream) if isinstance(stream, int) else stream)
+    n = sbf_num_shards(handle) * 32
+    mine = sbf_ipc_export_filter(handle)
+    handles = [None] * world
+    dist.all_gather_object(handles, mine, group=group)
+    peer_ptr = {p: sbf_ipc_open_filter(handles[p]) for p in range(world) if p != rank}
+    local = filter_tensor(handle)
+    launches = 0
+    try:
+        with torch.cuda.stream(st):
+            for a, slices in merge_plan(n, world, window_bytes):
+                st.synchronize()
+                dist.barrier(group=group)                       # every rank's inserts (or previous window) are done
+                lo, hi = slices[rank]
+                if hi > lo:
+                    sbf_or_peers_range_device(handle, a + lo, [peer_ptr[p] + a + lo for p in peer_ptr], hi - lo, st)
+                    launches += 1
+                st.synchronize()
+                dist.barrier(group=group)                       # all slices reduced: gather them
+                for p, (plo, phi) in enumerate(slices):
+                    if p != rank and phi > plo:
+                        src = torch.as_tensor(DevicePtrView(peer_ptr[p] + a + plo, phi - plo), device="cuda")
+                        local[a + plo:a + phi].copy_(src, non_blocking=True)
+            st.synchronize()
+            dist.barrier(group=group)                           # nobody unmaps while a peer still reads
+    finally:
+        for p in peer_ptr.values():
+            sbf_ipc_close_filter(p)
+    return launches

@@ -282,6 +282,34 @@ def test_import_export_or_roundtrip():
         assert np.array_equal(fb.export_bits(), merged)
 
 
+@pytest.mark.parametrize("world,window", [(2, 1 << 28), (3, 40_000), (5, 9_999)])
+def test_replica_merge_on_one_device(world, window):
+    """The multi-GPU exchange's plan and kernels on ONE device: `world` replicas filled from a partition of the batch,
+    merged with replicas.merge_local_replicas (sbf_or_peers_range_device per slice, then the gather copies) — every
+    replica must equal the oracle's single filter.  Windows smaller than the filter, a ragged last window, slices of
+    unequal length."""
+    from paper_2606_24417_b200 import replicas
+    seq = seqgen.markov(31, 5, 0.41, 400_000)
+    seq[100_000:100_300] = ord("N")
+    o = oracle.OracleSBF(num_bits=1 << 21, **DEFAULT)
+    o.insert_records(seq, threads=True)
+    fs = [sbf.SuperBloomFilter(num_bits=1 << 21, **DEFAULT) for _ in range(world)]
+    try:
+        for r, f in enumerate(fs):
+            a, e = replicas.partition_positions(seq.size, DEFAULT["k"], world, r)
+            gpu_insert(f, seq[a:e])
+        n = replicas.merge_local_replicas([f.handle for f in fs], window_bytes=window)
+        torch.cuda.synchronize()
+        assert n >= world
+        want = o.export_bits()
+        for r, f in enumerate(fs):
+            assert np.array_equal(f.export_bits(), want), "replica %d differs from the single-rank filter" % r
+    finally:
+        for f in fs:
+            f.close()
+    o.close()
+
+
 def test_host_facing_calls_match_device_facing():
     """The host-facing forms (chunked staging) give the same filter, bitmap and counts."""
     w = seqgen.config2(scale=0.05)
