@@ -35,6 +35,9 @@
 #ifndef SBF_FMA_SIGMA
 #define SBF_FMA_SIGMA 0   // sigma's final shift as a multiply-high by 2^P (fma pipe; measured: no gain)
 #endif
+#ifndef SBF_CPASYNC_L2_64B
+#define SBF_CPASYNC_L2_64B 1 // query staging: cp.async with the .L2::64B prefetch-size hint (a miss then pulls 64 B from DRAM instead of 128 B: measured DRAM reads -44 %, same time)
+#endif
 #ifndef SBF_PRED_RELOAD
 #define SBF_PRED_RELOAD 1 // query: reload the shard registers with two predicated LDS.128 instead of a divergent branch
 #endif
@@ -57,6 +60,10 @@ constexpr uint64_t kMultF = 0xD6E8FEB86659FD93ull;
 // ---- launch geometry ---------------------------------------------------------------------
 constexpr int kChunk = 128;     // most k-mer start positions walked by one thread of stream_kernel (StreamParams::chunk_blocks * 16)
 constexpr int kStreamTPB = 128; // threads per CTA of stream_kernel
+#ifndef SBF_REC_TPB
+#define SBF_REC_TPB 128
+#endif
+constexpr int kRecTPB = SBF_REC_TPB; // threads per CTA of stream_rec_kernel
 constexpr int kPadWords = 16;   // zero / all-invalid words appended to the packed sequence and its mask
 
 struct StreamParams {
@@ -472,8 +479,13 @@ static_assert(kLA >= 1 && 16 % kNS == 0, "staging needs a look-ahead of 1, 3, 7 
 __device__ __forceinline__ void cp_async_shard(uint4 *smem_lo, uint4 *smem_hi, const uint64_t *g)
 {
     uint32_t a = (uint32_t)__cvta_generic_to_shared(smem_lo), b = (uint32_t)__cvta_generic_to_shared(smem_hi);
+#if SBF_CPASYNC_L2_64B
+    asm volatile("cp.async.cg.shared.global.L2::64B [%0], [%1], 16;" ::"r"(a), "l"(g) : "memory");
+    asm volatile("cp.async.cg.shared.global.L2::64B [%0], [%1], 16;" ::"r"(b), "l"(g + 2) : "memory");
+#else
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(a), "l"(g) : "memory");
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(b), "l"(g + 2) : "memory");
+#endif
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -483,7 +495,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // of a new run's sector, the newest s-mer's masks, the k-mer test of k-mer q.  Validity plays no part here: a
 // position without a valid k-mer computes on whatever symbols are there (its shard index is still in range) and its
 // result bit is cleared from V afterwards, 16 positions at a time.
-template <int K, int M, int S, int H>
+template <int K, int M, int S, int H, int TPB>
 struct QueryLane {
     static constexpr int WN = K - M + 1, Z = K - S, NW = H < 4 ? H : 4;
     SlidingMin<WN> smin;
@@ -522,7 +534,7 @@ struct QueryLane {
         const uint32_t shNew = sigma32(smin.template push<Q + WN - 1>(g_key(lmer<Q + WN - 1, M>(W), M)), prm.shard_shift);
         const bool start = FIRST || shNew != laPrev;
         if (start)
-            cp_async_shard(&stage[((Q % kNS) * 2) * kStreamTPB + threadIdx.x], &stage[((Q % kNS) * 2 + 1) * kStreamTPB + threadIdx.x],
+            cp_async_shard(&stage[((Q % kNS) * 2) * TPB + threadIdx.x], &stage[((Q % kNS) * 2 + 1) * TPB + threadIdx.x],
                            prm.filter + (uint64_t)shNew * 4);
         cp_async_commit();
         sb[Q % kNS] = start;
@@ -541,8 +553,8 @@ struct QueryLane {
         // BSSY/BSYNC paid) nearly always: wait unconditionally, load under a predicate
         cp_async_wait<kLA>();
         {
-            const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(&stage[((J % kNS) * 2) * kStreamTPB + threadIdx.x]);
-            const uint32_t a1 = (uint32_t)__cvta_generic_to_shared(&stage[((J % kNS) * 2 + 1) * kStreamTPB + threadIdx.x]);
+            const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(&stage[((J % kNS) * 2) * TPB + threadIdx.x]);
+            const uint32_t a1 = (uint32_t)__cvta_generic_to_shared(&stage[((J % kNS) * 2 + 1) * TPB + threadIdx.x]);
             asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %8, 0;\n\t"
                          "@p ld.shared.v4.u32 {%0,%1,%2,%3}, [%9];\n\t@p ld.shared.v4.u32 {%4,%5,%6,%7}, [%10];\n\t}"
                          : "+r"(sh32[0]), "+r"(sh32[1]), "+r"(sh32[2]), "+r"(sh32[3]), "+r"(sh32[4]), "+r"(sh32[5]), "+r"(sh32[6]),
@@ -553,8 +565,8 @@ struct QueryLane {
 #else
         if (sb[J % kNS]) {
             cp_async_wait<kLA>();
-            const uint4 lo = stage[((J % kNS) * 2) * kStreamTPB + threadIdx.x];
-            const uint4 hi = stage[((J % kNS) * 2 + 1) * kStreamTPB + threadIdx.x];
+            const uint4 lo = stage[((J % kNS) * 2) * TPB + threadIdx.x];
+            const uint4 hi = stage[((J % kNS) * 2 + 1) * TPB + threadIdx.x];
             sh32[0] = lo.x; sh32[1] = lo.y; sh32[2] = lo.z; sh32[3] = lo.w;
             sh32[4] = hi.x; sh32[5] = hi.y; sh32[6] = hi.z; sh32[7] = hi.w;
         }
@@ -685,7 +697,7 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
         }
         if constexpr (TMA_FLUSH) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); // slots intact until read
     } else {
-        QueryLane<K, M, S, H> ql;
+        QueryLane<K, M, S, H, kStreamTPB> ql;
         ql.prologue(W, prm, stage);
         uint32_t res = 0;
         for (int b = 0; b < prm.chunk_blocks; ++b) {
@@ -723,9 +735,13 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
 // kernels, launched right after, redo the whole batch (they do nothing while the flag is clear).
 // =============================================================================================
 template <int K, int M, int S, int H>
-__global__ void __launch_bounds__(kStreamTPB, SBF_MINB_R) stream_rec_kernel(const StreamParams prm)
+#ifdef SBF_REC_MAXREG
+__global__ void __maxnreg__(SBF_REC_MAXREG) stream_rec_kernel(const StreamParams prm)
+#else
+__global__ void __launch_bounds__(kRecTPB, SBF_MINB_R) stream_rec_kernel(const StreamParams prm)
+#endif
 {
-    __shared__ uint4 stage[kNS * 2 * kStreamTPB];
+    __shared__ uint4 stage[kNS * 2 * kRecTPB];
 
     const uint64_t r = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= prm.n_rec) return;
@@ -753,7 +769,7 @@ __global__ void __launch_bounds__(kStreamTPB, SBF_MINB_R) stream_rec_kernel(cons
     }
     uint32_t vcur = (uint32_t)__ldg(vw) | ((uint32_t)__ldg(vw + 1) << 16); // V bits of the symbols from 16*(a>>4) on
 
-    QueryLane<K, M, S, H> ql;
+    QueryLane<K, M, S, H, kRecTPB> ql;
     ql.prologue(W, prm, stage);
 
     // result bits leave through a 64-bit buffer aligned to the bitmap's words

@@ -35,8 +35,8 @@ template <int K, int M, int S, int H>
 cudaError_t launch_stream_rec(const StreamParams &prm, cudaStream_t stream)
 {
     if (prm.n_rec == 0) return cudaSuccess;
-    const uint64_t blocks = (prm.n_rec + kStreamTPB - 1) / kStreamTPB;
-    stream_rec_kernel<K, M, S, H><<<(unsigned)blocks, kStreamTPB, 0, stream>>>(prm);
+    const uint64_t blocks = (prm.n_rec + kRecTPB - 1) / kRecTPB;
+    stream_rec_kernel<K, M, S, H><<<(unsigned)blocks, kRecTPB, 0, stream>>>(prm);
     return cudaGetLastError();
 }
 
