@@ -58,6 +58,9 @@ typedef enum sbf_status {
  *   per shard, 32 bytes per shard, 32-byte aligned (one L2 sector per shard).
  *   (k,m,s,H) combinations compiled as specialised streaming kernels run those; every
  *   other legal combination runs a runtime-parameter CUDA kernel (same bits, slower).
+ *   Side effect on the DEVICE (not only this handle): when the filter is small enough to be kept in L2 (a7), the
+ *   call raises cudaLimitPersistingL2CacheSize to the device maximum if it is lower, and every later call on this
+ *   handle sets an access-policy window for the filter on the stream it is given.
  *   Returns NULL on error.
  */
 sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits);

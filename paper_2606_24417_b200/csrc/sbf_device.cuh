@@ -38,6 +38,9 @@
 #ifndef SBF_CPASYNC_L2_64B
 #define SBF_CPASYNC_L2_64B 1 // query staging: cp.async with the .L2::64B prefetch-size hint (a miss then pulls 64 B from DRAM instead of 128 B: measured DRAM reads -44 %, same time)
 #endif
+#ifndef SBF_EARLY_RELOAD
+#define SBF_EARLY_RELOAD 0 // query: reload the shard registers at the top of a step (measured: no gain, the scheduler already hides the LDS)
+#endif
 #ifndef SBF_PRED_RELOAD
 #define SBF_PRED_RELOAD 1 // query: reload the shard registers with two predicated LDS.128 instead of a divergent branch
 #endif
@@ -45,7 +48,7 @@
 #define SBF_MINB_I 5 // insert: CTAs per SM the register budget is cut for (5 x 128 threads -> 96 registers)
 #endif
 #ifndef SBF_MINB_Q
-#define SBF_MINB_Q 5 // query: 5 x 128 threads -> 96 registers
+#define SBF_MINB_Q 4 // chunk-mode query: 4 x 128 threads -> 128 registers (5 -> 96 registers spills: 0.333 vs 0.328 ms per 100 Mbp)
 #endif
 
 namespace sbfk {
@@ -544,14 +547,18 @@ struct QueryLane {
     template <int J>
     __device__ __forceinline__ bool step(const uint32_t (&W)[4], const StreamParams &prm, uint4 *stage)
     {
-        this->template look<J + kLA, false>(W, prm, stage);
-        uint64_t Mn[NW];
-        expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
-        // a6: if a run starts here, its sector was staged kLA positions ago: take it into the shard registers
+        // a6: if a run starts here, its sector was staged kLA positions ago: take it into the shard registers.
 #if SBF_PRED_RELOAD
-        // almost every warp has SOME lane starting a run at any given position, so a branch would be taken (and its
-        // BSSY/BSYNC paid) nearly always: wait unconditionally, load under a predicate
+        // Almost every warp has SOME lane starting a run at any given position, so a branch would be taken (and its
+        // BSSY/BSYNC paid) nearly always: wait unconditionally, load under a predicate.  SBF_EARLY_RELOAD: do it FIRST
+        // in the step (before this step's own look-ahead commits its group, hence wait_group kLA - 1), so that the
+        // shared-memory latency hides behind the minimizer and hash work instead of in front of the test.
+#if SBF_EARLY_RELOAD
+        cp_async_wait<kLA - 1>();
+#else
+        this->template look<J + kLA, false>(W, prm, stage);
         cp_async_wait<kLA>();
+#endif
         {
             const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(&stage[((J % kNS) * 2) * TPB + threadIdx.x]);
             const uint32_t a1 = (uint32_t)__cvta_generic_to_shared(&stage[((J % kNS) * 2 + 1) * TPB + threadIdx.x]);
@@ -562,7 +569,11 @@ struct QueryLane {
                          : "r"((uint32_t)sb[J % kNS]), "r"(a0), "r"(a1)
                          : "memory");
         }
+#if SBF_EARLY_RELOAD
+        this->template look<J + kLA, false>(W, prm, stage);
+#endif
 #else
+        this->template look<J + kLA, false>(W, prm, stage);
         if (sb[J % kNS]) {
             cp_async_wait<kLA>();
             const uint4 lo = stage[((J % kNS) * 2) * TPB + threadIdx.x];
@@ -571,6 +582,8 @@ struct QueryLane {
             sh32[4] = hi.x; sh32[5] = hi.y; sh32[6] = hi.z; sh32[7] = hi.w;
         }
 #endif
+        uint64_t Mn[NW];
+        expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
         const uint64_t shard[4] = {((uint64_t)sh32[1] << 32) | sh32[0], ((uint64_t)sh32[3] << 32) | sh32[2],
                                    ((uint64_t)sh32[5] << 32) | sh32[4], ((uint64_t)sh32[7] << 32) | sh32[6]};
         return sor.template push_test<J + Z>(Mn, shard) == 0;
