@@ -69,7 +69,8 @@ sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits);
  * sbf_create_ex — the same for any of the paper's three alphabets and for packed k-mers wider than one 64-bit
  * word ("multiword"); readings A19-A22 of DESIGN.md §3.  k * symbol_bits <= 128:
  *   SBF_ALPHABET_DNA          2 bits, A C G T either case, k <= 64 (sbf_create is this alphabet; k <= 32 runs the
- *                             specialised / runtime kernels above, 33 <= k <= 64 the wide kernel)
+ *                             specialised / runtime kernels above; 33 <= k <= 64 runs specialised streaming kernels
+ *                             where an instance is compiled — e.g. (63,40,60,4), (51,31,48,4) — else the wide kernel)
  *   SBF_ALPHABET_PROTEIN      5 bits, the 26 letters either case (code = letter - 'A'), k <= 25
  *   SBF_ALPHABET_DNA_TRIPLET  6 bits, one symbol = three DNA bases (code = 16 c0 + 4 c1 + c2), k <= 21; symbols sit at
  *                             multiples of three bytes from the start of their record; k, m, s count SYMBOLS

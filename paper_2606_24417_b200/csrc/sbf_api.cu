@@ -450,7 +450,8 @@ sbf_t *sbf_create_ex(int k, int m, int s, int H, uint64_t num_bits, int alphabet
     }
     f->k = k; f->m = m; f->s = s; f->H = H; f->P = P; f->device = dev;
     f->alphabet = alphabet; f->sym_bits = sym_bits; f->sym_bytes = alphabet == SBF_ALPHABET_DNA_TRIPLET ? 3 : 1;
-    f->wide = alphabet != SBF_ALPHABET_DNA || k > 32;
+    // DNA with 33 <= k <= 64 has specialised streaming instances too (folded wide windows, A21); without one: wide_kernel
+    f->wide = alphabet != SBF_ALPHABET_DNA || (k > 32 && find_entry(k, m, s, H) == nullptr);
     f->num_shards = shards;
     f->host_chunk = kHostChunkDefault;
     f->tma_flush = shards * 32 >= kTmaFlushMinBytes;

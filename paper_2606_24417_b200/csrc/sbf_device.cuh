@@ -237,36 +237,48 @@ __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ s
         word[w >> 2] |= c8 << (24 - 8 * (w & 3));
         inv |= i4 << (4 * w);
     }
-    // B of the next 32 symbols: the next thread's word through shared memory; only the last thread of the CTA has to
-    // classify them itself (a per-warp exchange would send one lane in 32 down that divergent path)
+    // B of the next 32 (k > 33: 64) symbols: the following threads' words through shared memory; only the last thread(s)
+    // of the CTA classify them themselves (a per-warp exchange would send one lane in 32 down that divergent path)
     __shared__ uint32_t s_inv[256];
     s_inv[threadIdx.x] = inv;
     __syncthreads();
-    uint32_t nxt;
-    if (threadIdx.x + 1 < blockDim.x) {
-        nxt = s_inv[threadIdx.x + 1];
-    } else {
-        load32(seq, b0 + 32, len, aligned16, v);
-        nxt = 0;
+    auto inv_ahead = [&](unsigned d) -> uint32_t { // B bits of symbols [b0 + 32 d, b0 + 32 d + 32)
+        if (threadIdx.x + d < blockDim.x) return s_inv[threadIdx.x + d];
+        uint32_t vv[8], r = 0;
+        load32(seq, b0 + 32ull * d, len, aligned16, vv);
 #pragma unroll
         for (int w = 0; w < 8; ++w) {
             uint32_t i4;
-            (void)pack4(v[w], i4);
-            nxt |= i4 << (4 * w);
+            (void)pack4(vv[w], i4);
+            r |= i4 << (4 * w);
         }
-    }
+        return r;
+    };
+    const uint32_t nxt = inv_ahead(1);
     // V = OR of k consecutive B bits, by doubling: after the loop bit j of y covers B[j .. j+c-1], c the largest power
     // of two <= k; one more step with the remainder closes the window (k - c <= c)
-    uint64_t y = (uint64_t)inv | ((uint64_t)nxt << 32);
-    if (__any_sync(0xFFFFFFFFu, y != 0)) { // almost every warp sees only valid symbols: V = 0 without the doubling
+    uint32_t g;
+    if (k <= 33) {
+        uint64_t y = (uint64_t)inv | ((uint64_t)nxt << 32);
+        if (__any_sync(0xFFFFFFFFu, y != 0)) { // almost every warp sees only valid symbols: V = 0 without the doubling
+            int c = 1;
+            while (2 * c <= k) {
+                y |= y >> c;
+                c *= 2;
+            }
+            if (c < k) y |= y >> (k - c);
+        }
+        g = (uint32_t)y;
+    } else { // 33 < k <= 64: the window reaches into the third word
+        unsigned __int128 y = (unsigned __int128)inv | ((unsigned __int128)nxt << 32) | ((unsigned __int128)inv_ahead(2) << 64);
         int c = 1;
         while (2 * c <= k) {
             y |= y >> c;
             c *= 2;
         }
         if (c < k) y |= y >> (k - c);
+        g = (uint32_t)y;
     }
-    const uint32_t g = (uint32_t)y;
     if (2 * i + 1 < n_words_total) {
         *reinterpret_cast<uint2 *>(packed + 2 * i) = make_uint2(word[0], word[1]);
         *reinterpret_cast<uint32_t *>(vmask + 2 * i) = g;
@@ -288,49 +300,60 @@ __global__ void __launch_bounds__(256) mark_ends_kernel(const uint64_t *__restri
         const uint64_t e = offsets[r];
         if (k < 2 || e == 0 || e > total) continue;
         const uint64_t lo = e >= (uint64_t)(k - 1) ? e - (uint64_t)(k - 1) : 0;
-        const uint64_t mask = (((uint64_t)1 << (e - lo)) - 1) << (lo & 31); // at most 31 bits, spanning at most two words
+        // at most k - 1 <= 63 bits starting at bit (lo & 31): at most three words
+        const unsigned __int128 mask = ((((unsigned __int128)1) << (e - lo)) - 1) << (lo & 31);
         atomicOr(&vmask32[lo >> 5], (uint32_t)mask);
-        if (mask >> 32) atomicOr(&vmask32[(lo >> 5) + 1], (uint32_t)(mask >> 32));
+        if ((uint32_t)(mask >> 32)) atomicOr(&vmask32[(lo >> 5) + 1], (uint32_t)(mask >> 32));
+        if ((uint32_t)(mask >> 64)) atomicOr(&vmask32[(lo >> 5) + 2], (uint32_t)(mask >> 64));
     }
 }
 
 #endif // SBF_DEFINE_AUX_KERNELS
 
 // =============================================================================================
-// Window access for stream_kernel.  W[0..3] hold 64 consecutive symbols (W[0] first, first symbol
-// in the top bits).  lmer<O,N>(W) = the N-mer starting O symbols into the window, as Sub() of the
-// paper's packed k-mer (first base most significant).  All shifts are immediates.
+// Window access for stream_kernel.  W[0..NWIN-1] hold 16 * NWIN consecutive symbols (W[0] first, first symbol in the
+// top bits).  lmer<O,N>(W) = the N-mer starting O symbols into the window, as Sub() of the paper's packed k-mer (first
+// base most significant); an N-mer wider than 64 bits (N > 32: k-mers of 33..64 bases, A20) comes back folded to
+// 64 bits as A21 prescribes (its last 32 symbols XOR the rotated golden-ratio multiple of the symbols before them).
+// All shifts are immediates.  NWIN = 4 up to k = 42, 5 up to k = 58, 6 up to k = 64 (kWinOf).
 // =============================================================================================
-constexpr int kWin = 4; // 32-bit words in the register window
+__host__ __device__ constexpr int kWinOf(int K) { return (K + 22 + 15) / 16 < 4 ? 4 : (K + 22 + 15) / 16; } // 15 + look-ahead 7 + k symbols
 
-template <int Q, int NB>
-__device__ __forceinline__ uint32_t field_win(const uint32_t (&W)[kWin])
+template <int Q, int NB, int NWIN>
+__device__ __forceinline__ uint32_t field_win(const uint32_t (&W)[NWIN])
 {
-    // bits [Q, Q+NB) of the window, counted from the least significant bit of W[kWin-1]
-    static_assert(Q >= 0 && NB >= 1 && NB <= 32 && Q + NB <= 32 * kWin, "field outside the register window");
+    // bits [Q, Q+NB) of the window, counted from the least significant bit of W[NWIN-1]
+    static_assert(Q >= 0 && NB >= 1 && NB <= 32 && Q + NB <= 32 * NWIN, "field outside the register window");
     constexpr int idx = Q / 32, sh = Q % 32;
-    uint32_t lo = W[kWin - 1 - idx];
+    uint32_t lo = W[NWIN - 1 - idx];
     uint32_t v;
     if constexpr (sh == 0) {
         v = lo;
     } else if constexpr (sh + NB <= 32) {
         v = lo >> sh;
     } else {
-        v = __funnelshift_r(lo, W[kWin - 2 - idx], sh);
+        v = __funnelshift_r(lo, W[NWIN - 2 - idx], sh);
     }
     if constexpr (NB < 32 && !(sh + NB == 32)) v &= (1u << NB) - 1u;
     return v;
 }
 
-template <int O, int N>
-__device__ __forceinline__ uint64_t lmer(const uint32_t (&W)[kWin])
+template <int O, int N, int NWIN>
+__device__ __forceinline__ uint64_t lmer(const uint32_t (&W)[NWIN])
 {
-    constexpr int Q = 32 * kWin - 2 * O - 2 * N;
-    constexpr int nb = 2 * N;
-    uint32_t lo = field_win<Q, (nb < 32 ? nb : 32)>(W);
-    uint32_t hi = 0;
-    if constexpr (nb > 32) hi = field_win<Q + 32, nb - 32>(W);
-    return ((uint64_t)hi << 32) | lo;
+    if constexpr (N <= 32) {
+        constexpr int Q = 32 * NWIN - 2 * O - 2 * N;
+        constexpr int nb = 2 * N;
+        uint32_t lo = field_win<Q, (nb < 32 ? nb : 32)>(W);
+        uint32_t hi = 0;
+        if constexpr (nb > 32) hi = field_win<Q + 32, nb - 32>(W);
+        return ((uint64_t)hi << 32) | lo;
+    } else {
+        const uint64_t lo = lmer<O + (N - 32), 32>(W); // the last 32 symbols: the low 64 bits of the window
+        const uint64_t hi = lmer<O, N - 32>(W);        // the symbols before them: the bits above
+        const uint64_t t = hi * kGold64;
+        return lo ^ ((t << 32) | (t >> 32));
+    }
 }
 
 __device__ __forceinline__ uint32_t min3u(uint32_t a, uint32_t b, uint32_t c) { return min(min(a, b), c); }
@@ -500,7 +523,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 // result bit is cleared from V afterwards, 16 positions at a time.
 template <int K, int M, int S, int H, int TPB>
 struct QueryLane {
-    static constexpr int WN = K - M + 1, Z = K - S, NW = H < 4 ? H : 4;
+    static constexpr int WN = K - M + 1, Z = K - S, NW = H < 4 ? H : 4, NWIN = kWinOf(K);
     SlidingMin<WN> smin;
     SlidingOr<Z + 1, NW> sor;
     uint32_t sh32[8]; // the current shard's four sector words as 32-bit halves (little-endian)
@@ -508,7 +531,7 @@ struct QueryLane {
     bool sb[kNS]; // sb[q mod kNS]: a run starts at k-mer q (its sector is in staging slot q mod kNS)
 
     // keys of the first WN-1 m-mers, masks of the first Z s-mers, shards of the first kLA k-mers
-    __device__ __forceinline__ void prologue(const uint32_t (&W)[4], const StreamParams &prm, uint4 *stage)
+    __device__ __forceinline__ void prologue(const uint32_t (&W)[NWIN], const StreamParams &prm, uint4 *stage)
     {
 #pragma unroll
         for (int i = 0; i < 16; ++i) { smin.g[i] = 0; smin.c3[i] = 0; smin.c9[i] = 0; }
@@ -532,7 +555,7 @@ struct QueryLane {
     }
     // k-mer Q (relative to the window): its shard; a change of shard starts a run and stages that sector
     template <int Q, bool FIRST>
-    __device__ __forceinline__ void look(const uint32_t (&W)[4], const StreamParams &prm, uint4 *stage)
+    __device__ __forceinline__ void look(const uint32_t (&W)[NWIN], const StreamParams &prm, uint4 *stage)
     {
         const uint32_t shNew = sigma32(smin.template push<Q + WN - 1>(g_key(lmer<Q + WN - 1, M>(W), M)), prm.shard_shift);
         const bool start = FIRST || shNew != laPrev;
@@ -545,7 +568,7 @@ struct QueryLane {
     }
     // k-mer J of the current 16-position block: returns true iff all its H(k-s+1) bits are set in its shard
     template <int J>
-    __device__ __forceinline__ bool step(const uint32_t (&W)[4], const StreamParams &prm, uint4 *stage)
+    __device__ __forceinline__ bool step(const uint32_t (&W)[NWIN], const StreamParams &prm, uint4 *stage)
     {
         // a6: if a run starts here, its sector was staged kLA positions ago: take it into the shard registers.
 #if SBF_PRED_RELOAD
@@ -614,7 +637,8 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
     constexpr int Z = K - S;
     constexpr int NW = H < 4 ? H : 4;
     constexpr int RZ = ring_size(Z);
-    static_assert(K >= 1 && K <= 32 && M >= 1 && M <= K && S >= 1 && S <= K, "bad k/m/s");
+    constexpr int NWIN = kWinOf(K);
+    static_assert(K >= 1 && K <= 64 && M >= 1 && M <= K && S >= 1 && S <= K, "bad k/m/s");
     static_assert(Z <= 16, "stream kernel supports k-s <= 16");
     __shared__ uint4 stage[INSERT ? 1 : kNS * 2 * kStreamTPB];
     __shared__ ulonglong2 flush_slots[TMA_FLUSH ? kFlushSlots * kStreamTPB * 2 : 1];
@@ -631,7 +655,9 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
 
     const uint32_t *__restrict__ pw = prm.packed + (p0 >> 4);
     const uint16_t *__restrict__ vw = prm.vmask + (p0 >> 4);
-    uint32_t W[kWin] = {__ldg(pw), __ldg(pw + 1), __ldg(pw + 2), __ldg(pw + 3)};
+    uint32_t W[NWIN];
+#pragma unroll
+    for (int i = 0; i < NWIN; ++i) W[i] = __ldg(pw + i);
 
     if constexpr (INSERT) {
         SlidingMin<WN> smin;
@@ -656,7 +682,7 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
         uint32_t prevShard = 0;
         bool prevInval = true;
         for (int b = 0; b < prm.chunk_blocks; ++b) {
-            const uint32_t wnext = __ldg(pw + b + 4);
+            const uint32_t wnext = __ldg(pw + b + NWIN);
             const uint32_t v16 = __ldg(vw + b);
             static_for<0, 16>([&](auto jc) {
                 constexpr int J = decltype(jc)::value;
@@ -695,7 +721,9 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
 #pragma unroll
                 for (int q = 0; q < NW; ++q) Mh[(J + Z) % RZ][q] = Mn[q];
             });
-            W[0] = W[1]; W[1] = W[2]; W[2] = W[3]; W[3] = wnext;
+#pragma unroll
+            for (int i = 0; i + 1 < NWIN; ++i) W[i] = W[i + 1];
+            W[NWIN - 1] = wnext;
         }
         if (!prevInval) {
             uint64_t *dst = prm.filter + (uint64_t)prevShard * 4;
@@ -714,7 +742,7 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
         ql.prologue(W, prm, stage);
         uint32_t res = 0;
         for (int b = 0; b < prm.chunk_blocks; ++b) {
-            const uint32_t wnext = __ldg(pw + b + 4);
+            const uint32_t wnext = __ldg(pw + b + NWIN);
             const uint32_t v16 = __ldg(vw + b);
             uint32_t res16 = 0;
             static_for<0, 16>([&](auto jc) {
@@ -722,7 +750,9 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
                 if (ql.template step<J>(W, prm, stage)) res16 |= 1u << J;
             });
             res16 &= ~v16; // a1: positions without a valid k-mer answer false
-            W[0] = W[1]; W[1] = W[2]; W[2] = W[3]; W[3] = wnext;
+#pragma unroll
+            for (int i = 0; i + 1 < NWIN; ++i) W[i] = W[i + 1];
+            W[NWIN - 1] = wnext;
             res = (res >> 16) | (res16 << 16);
             if (b & 1) {
                 const uint64_t wi = (p0 >> 5) + (uint64_t)(b >> 1);
@@ -772,13 +802,16 @@ __global__ void __launch_bounds__(kRecTPB, SBF_MINB_R) stream_rec_kernel(const S
     const uint32_t *__restrict__ pw = prm.packed + (a >> 4);
     const uint16_t *__restrict__ vw = prm.vmask + (a >> 4);
     const uint32_t s2 = 2u * (uint32_t)(a & 15), s1 = (uint32_t)(a & 15);
+    constexpr int NWIN = kWinOf(K);
     uint32_t rawLast;
-    uint32_t W[kWin];
+    uint32_t W[NWIN];
     {
-        const uint32_t r0 = __ldg(pw), r1 = __ldg(pw + 1), r2 = __ldg(pw + 2), r3 = __ldg(pw + 3);
-        rawLast = __ldg(pw + 4);
-        W[0] = __funnelshift_l(r1, r0, s2); W[1] = __funnelshift_l(r2, r1, s2);
-        W[2] = __funnelshift_l(r3, r2, s2); W[3] = __funnelshift_l(rawLast, r3, s2);
+        uint32_t raw[NWIN + 1];
+#pragma unroll
+        for (int i = 0; i <= NWIN; ++i) raw[i] = __ldg(pw + i);
+#pragma unroll
+        for (int i = 0; i < NWIN; ++i) W[i] = __funnelshift_l(raw[i + 1], raw[i], s2);
+        rawLast = raw[NWIN];
     }
     uint32_t vcur = (uint32_t)__ldg(vw) | ((uint32_t)__ldg(vw + 1) << 16); // V bits of the symbols from 16*(a>>4) on
 
@@ -802,7 +835,7 @@ __global__ void __launch_bounds__(kRecTPB, SBF_MINB_R) stream_rec_kernel(const S
 
     const uint32_t nblk = (nk + 15) >> 4;
     for (uint32_t b = 0; b < nblk; ++b) {
-        const uint32_t rawNext = __ldg(pw + b + 5);
+        const uint32_t rawNext = __ldg(pw + b + NWIN + 1);
         const uint32_t vNext = __ldg(vw + b + 2);
         uint32_t res16 = 0;
         static_for<0, 8>([&](auto jc) {
@@ -814,7 +847,9 @@ __global__ void __launch_bounds__(kRecTPB, SBF_MINB_R) stream_rec_kernel(const S
                 constexpr int J = decltype(jc)::value;
                 if (ql.template step<J>(W, prm, stage)) res16 |= 1u << J;
             });
-        W[0] = W[1]; W[1] = W[2]; W[2] = W[3]; W[3] = __funnelshift_l(rawNext, rawLast, s2);
+#pragma unroll
+        for (int i = 0; i + 1 < NWIN; ++i) W[i] = W[i + 1];
+        W[NWIN - 1] = __funnelshift_l(rawNext, rawLast, s2);
         rawLast = rawNext;
         res16 &= ~(vcur >> s1) & 0xFFFFu;   // a1: V bits of these 16 positions (re-aligned like the window)
         vcur = (vcur >> 16) | (vNext << 16);

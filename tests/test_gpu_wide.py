@@ -41,12 +41,12 @@ def ragged_offsets(rng, total, mean):
     return np.concatenate(([0], np.cumsum(lens))).astype(np.uint64)
 
 
-def check(alphabet, k, m, s, H, num_bits, ins, ins_offs, q, q_offs):
+def check(alphabet, k, m, s, H, num_bits, ins, ins_offs, q, q_offs, specialized=False):
     o = oracle.OracleSBF(k, m, s, H, num_bits, alphabet=alphabet)
     n_ins = o.insert_records(ins, ins_offs, threads=True)
     assert n_ins > 0
     with sbf.SuperBloomFilter(k=k, m=m, s=s, H=H, num_bits=num_bits, alphabet=alphabet) as f:
-        assert not f.specialized and f.num_shards == o.num_shards
+        assert f.specialized == specialized and f.num_shards == o.num_shards
         d = dev(ins)
         if ins_offs is None:
             sbf.sbf_insert_seq(f.handle, d, d.numel())
@@ -156,3 +156,35 @@ def test_host_facing_calls_in_several_chunks(alphabet, k, m, s, H):
             wbm2, wc2, _ = o.query_records(q, None)
             assert np.array_equal(bm2, wbm2) and int(hits[0]) == int(wc2.sum())
         o.close(); o_seq.close()
+
+
+# DNA k-mers of 33..64 bases that have SPECIALISED streaming instances (csrc/sbf_inst_wide.cu): the thread-serial kernels
+# with a wider register window and folded (A21) m-mers / s-mers
+WIDE_SPECIALISED = [(63, 40, 60, 4), (51, 31, 48, 4), (47, 24, 44, 4), (33, 16, 30, 4), (64, 41, 64, 8)]
+
+
+@pytest.mark.parametrize("k,m,s,H", WIDE_SPECIALISED)
+def test_specialised_wide_k_instances(k, m, s, H):
+    """Insert (sequence: chunk mode; record batch: chunk mode + record-end marking with k-1 up to 63 bits), record-mode
+    query of 150-base reads, its fallback (one long record), chunk-mode query of a sequence — against the oracle's wide path."""
+    rng = np.random.default_rng(k)
+    w = seqgen.config3(scale=0.004)                                   # 1 Mbp with an N run
+    ins = w.insert_bases
+    ins[rng.integers(0, ins.size, 40)] = ord("N")
+    ins[7000:7400] |= 0x20
+    reads = w.read_batch(0, 6000)
+    offs = seqgen.fixed_offsets(6000, 150)
+    check(oracle.DNA, k, m, s, H, 1 << 24, ins, None, reads, offs, specialized=True)                  # record mode
+    lens = np.full(6000, 150, dtype=np.int64); lens[17] = 3000; lens[100:140] = rng.integers(0, 80, 40)
+    roffs = np.concatenate(([0], np.cumsum(lens))).astype(np.uint64)
+    q2 = np.concatenate((reads, seqgen.uniform(5, int(roffs[-1]) - reads.size))) if int(roffs[-1]) > reads.size else reads[:int(roffs[-1])].copy()
+    check(oracle.DNA, k, m, s, H, 1 << 24, ins, ragged_offsets(rng, ins.size, 4000), q2, roffs, specialized=True)  # fallback
+    check(oracle.DNA, k, m, s, H, 1 << 24, ins, None, reads, None, specialized=True)                  # chunk-mode query
+
+
+@pytest.mark.slow
+def test_specialised_k63_at_25_mbp():
+    k, m, s, H = 63, 40, 60, 4
+    w = seqgen.config3(scale=0.1)
+    reads = w.read_batch(0, 200_000)
+    check(oracle.DNA, k, m, s, H, 1 << 30, w.insert_bases, None, reads, seqgen.fixed_offsets(200_000, 150), specialized=True)
