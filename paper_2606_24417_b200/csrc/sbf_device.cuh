@@ -360,11 +360,17 @@ __device__ __forceinline__ uint32_t min3u(uint32_t a, uint32_t b, uint32_t c) { 
 
 // Sliding minimum of the last WN keys, streaming: keys arrive one per step, E = step phase (mod 16
 // is all that matters).  Levels c3 = min of the last 3, c9 = min of the last 9; the window of WN is
-// covered by two or three overlapping blocks (three-input minimum = VIMNMX3 on sm_100a).
+// covered by two or three overlapping blocks (three-input minimum = VIMNMX3 on sm_100a); above 24 keys (k-mers of more
+// than 32 bases with m near k/2) a fourth level keeps the minimum of the last 24 and joins it with an earlier one.
 template <int WN>
 struct SlidingMin {
-    static_assert(WN >= 1 && WN <= 24, "stream kernel supports k-m+1 <= 24");
-    uint32_t g[16], c3[16], c9[16];
+    static_assert(WN >= 1 && WN <= 39, "stream kernel supports k-m+1 <= 39");
+    uint32_t g[16], c3[16], c9[16], c24[16];
+    __device__ __forceinline__ void clear()
+    {
+#pragma unroll
+        for (int i = 0; i < 16; ++i) { g[i] = 0; c3[i] = 0; c9[i] = 0; c24[i] = 0; }
+    }
     template <int E>
     __device__ __forceinline__ uint32_t push(uint32_t gn)
     {
@@ -381,7 +387,12 @@ struct SlidingMin {
             uint32_t a9 = min3u(a3, c3[(E - 3) & 15], c3[(E - 6) & 15]);
             c9[s0] = a9;
             if constexpr (WN <= 18) return min(a9, c9[(E - (WN - 9)) & 15]);
-            else return min3u(a9, c9[(E - 9) & 15], c9[(E - (WN - 9)) & 15]);
+            else if constexpr (WN <= 24) return min3u(a9, c9[(E - 9) & 15], c9[(E - (WN - 9)) & 15]);
+            else {
+                const uint32_t a24 = min3u(a9, c9[(E - 9) & 15], c9[(E - 15) & 15]);
+                c24[s0] = a24;
+                return min(a24, c24[(E - (WN - 24)) & 15]);
+            }
         }
         return gn;
     }
@@ -533,8 +544,7 @@ struct QueryLane {
     // keys of the first WN-1 m-mers, masks of the first Z s-mers, shards of the first kLA k-mers
     __device__ __forceinline__ void prologue(const uint32_t (&W)[NWIN], const StreamParams &prm, uint4 *stage)
     {
-#pragma unroll
-        for (int i = 0; i < 16; ++i) { smin.g[i] = 0; smin.c3[i] = 0; smin.c9[i] = 0; }
+        smin.clear();
         sor.clear();
 #pragma unroll
         for (int q = 0; q < 8; ++q) sh32[q] = 0;
@@ -661,8 +671,7 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
 
     if constexpr (INSERT) {
         SlidingMin<WN> smin;
-#pragma unroll
-        for (int i = 0; i < 16; ++i) { smin.g[i] = 0; smin.c3[i] = 0; smin.c9[i] = 0; }
+        smin.clear();
         uint64_t Mh[RZ][NW]; // masks of the last k-s s-mers: what a new run shares with the k-mers before it
 #pragma unroll
         for (int i = 0; i < RZ; ++i)

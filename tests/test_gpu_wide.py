@@ -73,7 +73,7 @@ def check(alphabet, k, m, s, H, num_bits, ins, ins_offs, q, q_offs, specialized=
     o.close()
 
 
-CASES = [(oracle.DNA, 63, 31, 60, 4), (oracle.DNA, 64, 32, 64, 8), (oracle.DNA, 33, 16, 30, 12), (oracle.DNA, 47, 20, 40, 3),
+CASES = [(oracle.DNA, 63, 30, 59, 4), (oracle.DNA, 64, 32, 64, 8), (oracle.DNA, 33, 16, 30, 12), (oracle.DNA, 47, 20, 40, 3),
          (oracle.PROTEIN, 12, 6, 10, 4), (oracle.PROTEIN, 25, 7, 20, 4), (oracle.PROTEIN, 5, 2, 3, 2),
          (oracle.TRIPLET, 10, 5, 8, 4), (oracle.TRIPLET, 21, 9, 18, 6), (oracle.TRIPLET, 1, 1, 1, 1)]
 
@@ -160,7 +160,7 @@ def test_host_facing_calls_in_several_chunks(alphabet, k, m, s, H):
 
 # DNA k-mers of 33..64 bases that have SPECIALISED streaming instances (csrc/sbf_inst_wide.cu): the thread-serial kernels
 # with a wider register window and folded (A21) m-mers / s-mers
-WIDE_SPECIALISED = [(63, 40, 60, 4), (51, 31, 48, 4), (47, 24, 44, 4), (33, 16, 30, 4), (64, 41, 64, 8)]
+WIDE_SPECIALISED = [(63, 31, 60, 4), (51, 25, 48, 4), (63, 40, 60, 4), (51, 31, 48, 4), (47, 24, 44, 4), (33, 16, 30, 4), (64, 41, 64, 8)]
 
 
 @pytest.mark.parametrize("k,m,s,H", WIDE_SPECIALISED)
