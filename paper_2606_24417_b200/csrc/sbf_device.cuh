@@ -44,6 +44,12 @@
 #ifndef SBF_PRED_RELOAD
 #define SBF_PRED_RELOAD 1 // query: reload the shard registers with two predicated LDS.128 instead of a divergent branch
 #endif
+#ifndef SBF_GATHER
+#define SBF_GATHER 1 // query: byte-gather sliding test (SlidingGather) instead of 256-bit masks where it applies (H <= 4, k-s+1 in {1,2,4,8})
+#endif
+#ifndef SBF_GATHER_FMA_SHIFT
+#define SBF_GATHER_FMA_SHIFT 0 // SlidingGather: right shifts of the y fields as multiply-high (fma pipe)
+#endif
 #ifndef SBF_MINB_I
 #define SBF_MINB_I 5 // insert: CTAs per SM the register budget is cut for (5 x 128 threads -> 96 registers)
 #endif
@@ -448,6 +454,111 @@ struct SlidingOr {
     }
 };
 
+// Sliding Findere test WITHOUT 256-bit masks (query, H <= 4, k-s+1 in {1, 2, 4, 8}).  A bit position B(h,i) of sector
+// word q = i is (byte y = B >> 3, bit z = B & 7).  Per word q the thread keeps, for the last WO s-mers (ring slot
+// r = s-mer index mod WO, four slots per register):
+//   S[q] : four selector nibbles, nibble r = y of slot r   -> ONE byte permute G = PRMT(word q lo, word q hi, S[q])
+//          gathers, from the CURRENT shard, the byte each of the four s-mers must hit in word q;
+//   T[q] : four bytes, byte r = 1 << z of slot r           -> T[q] & ~G = bits of word q the k-mer misses.
+// Nothing here depends on the shard, so a shard change costs nothing (the gather always reads the current shard
+// registers), exactly like the mask form — but the state is 2 registers per word instead of ~6, and a position costs
+// ~21 alu-pipe instructions instead of ~37 (8 variable 64-bit shifts for the one-hot masks and 24 LOP3 for the sliding
+// OR and the AND-NOT over eight 32-bit halves are gone).  New s-mer, slot r: the y fields go into nibble r of S[q]
+// with one shift and one masked insert (LOP3) per word; the four z fields are packed into selector nibbles
+// (PRMT + mask + one multiply-add-high on the fma pipe), one table PRMT turns them into four one-hot bytes, and one
+// PRMT per word puts byte q of that into byte r of T[q].
+// prmt.b32 as is (__byte_perm would first AND the selector with 0x7777: one more LOP3 per use); selector nibbles must be 0..7
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel)
+{
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
+    return d;
+}
+// (a & mask) | (b & ~mask) as ONE LOP3 (written out, the compiler spends two: it sees two different constants)
+__device__ __forceinline__ uint32_t bitsel(uint32_t a, uint32_t b, uint32_t mask)
+{
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0xE4;" : "=r"(d) : "r"(a), "r"(b), "r"(mask));
+    return d;
+}
+
+template <int WO, int H>
+struct SlidingGather {
+    static_assert(H >= 1 && H <= 4 && (WO == 1 || WO == 2 || WO == 4 || WO == 8), "gather form: H <= 4, k-s+1 in {1,2,4,8}");
+    static constexpr int NW = H, Wd = 64 / H, NSET = WO > 4 ? 2 : 1;
+    uint32_t S[NSET][NW], T[NSET][NW];
+    __device__ __forceinline__ void clear()
+    {
+#pragma unroll
+        for (int a = 0; a < NSET; ++a)
+#pragma unroll
+            for (int q = 0; q < NW; ++q) { S[a][q] = 0; T[a][q] = 0; }
+    }
+    template <int SH>
+    __device__ __forceinline__ static uint32_t shift_to(uint32_t x) // x >> SH (SH > 0) or x << -SH
+    {
+        if constexpr (SH == 0) return x;
+        else if constexpr (SH > 0) {
+#if SBF_GATHER_FMA_SHIFT
+            return __umulhi(x, 1u << (32 - SH));
+#else
+            return x >> SH;
+#endif
+        } else return x << (-SH);
+    }
+    // the four (H) z fields of hash h as clean selector nibbles, nibble q = z of word q
+    __device__ __forceinline__ static uint32_t z_nibbles(uint32_t lo, uint32_t hi)
+    {
+        if constexpr (H == 4) { // fields at bits 0, 16 (lo), 0, 16 (hi): bytes (lo.b0, hi.b0, lo.b2, hi.b2), then byte 2 -> nibble 1, byte 1 -> nibble 2
+            const uint32_t pm = prmt(lo, hi, 0x6240u) & 0x07070707u;
+            uint32_t zs;
+            asm("mad.hi.u32 %0, %1, %2, %1;" : "=r"(zs) : "r"(pm), "r"(1u << 20)); // pm | (pm >> 12); bits above 15 are ignored by PRMT
+            return zs;
+        } else if constexpr (H == 2) { // fields at bit 0 of lo and of hi
+            return (lo & 7u) | ((hi & 7u) << 4);
+        } else if constexpr (H == 1) {
+            return lo & 7u;
+        } else {
+            uint32_t zs = 0;
+            static_for<0, H>([&](auto qc) {
+                constexpr int q = decltype(qc)::value, off = q * Wd;
+                zs |= (((off < 32 ? lo : hi) >> (off % 32)) & 7u) << (4 * q);
+            });
+            return zs;
+        }
+    }
+    template <int E>
+    __device__ __forceinline__ void push(uint64_t h)
+    {
+        constexpr int r = E % WO, a = r / 4, rr = r % 4;
+        const uint32_t lo = (uint32_t)h, hi = (uint32_t)(h >> 32);
+        const uint32_t onehot = prmt(0x08040201u, 0x80402010u, z_nibbles(lo, hi)); // byte q = 1 << z of word q
+        static_for<0, NW>([&](auto qc) {
+            constexpr int q = decltype(qc)::value, off = q * Wd;
+            static_assert(off % 32 + 6 <= 32, "a 6-bit slice straddles the halves of the hash");
+            constexpr uint32_t nib = 7u << (4 * rr);
+            const uint32_t y = shift_to<off % 32 + 3 - 4 * rr>(off < 32 ? lo : hi); // y field moved to nibble rr, junk around it
+            S[a][q] = bitsel(y, S[a][q], nib);
+            constexpr uint32_t keep = 0x3210u & ~(0xFu << (4 * rr)); // T[q] bytes stay, byte rr <- onehot byte q
+            T[a][q] = prmt(T[a][q], onehot, keep | ((uint32_t)(4 + q) << (4 * rr)));
+        });
+    }
+    // bits of the k-mer's H * WO positions that are NOT set in the shard (0 = present); sh32 = the sector as 8 halves
+    template <int E>
+    __device__ __forceinline__ uint32_t push_test(uint64_t h, const uint32_t (&sh32)[8])
+    {
+        push<E>(h);
+        uint32_t miss = 0;
+#pragma unroll
+        for (int a = 0; a < NSET; ++a)
+#pragma unroll
+            for (int q = 0; q < NW; ++q) miss |= T[a][q] & ~prmt(sh32[2 * q], sh32[2 * q + 1], S[a][q]);
+        return miss;
+    }
+};
+template <int WO, int H>
+constexpr bool gather_form() { return SBF_GATHER != 0 && H <= 4 && (WO == 1 || WO == 2 || WO == 4 || WO == 8); }
+
 // 1 << b for b in [0, 64) as two 32-bit halves.  SBF_FMA_ONEHOT: one shift on the alu pipe (1 << (b & 31)), the
 // half it belongs to picked by multiplications (b >> 5 as a multiply-high, then x * {0,1} and x - y as IMADs), which
 // issue on the fma pipe — the stream kernels are bound by the alu pipe, the fma pipe is two thirds idle.
@@ -535,8 +646,9 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 template <int K, int M, int S, int H, int TPB>
 struct QueryLane {
     static constexpr int WN = K - M + 1, Z = K - S, NW = H < 4 ? H : 4, NWIN = kWinOf(K);
+    static constexpr bool GATHER = gather_form<Z + 1, H>();
     SlidingMin<WN> smin;
-    SlidingOr<Z + 1, NW> sor;
+    std::conditional_t<GATHER, SlidingGather<GATHER ? Z + 1 : 1, GATHER ? H : 1>, SlidingOr<Z + 1, NW>> sor;
     uint32_t sh32[8]; // the current shard's four sector words as 32-bit halves (little-endian)
     uint32_t laPrev;
     bool sb[kNS]; // sb[q mod kNS]: a run starts at k-mer q (its sector is in staging slot q mod kNS)
@@ -557,9 +669,13 @@ struct QueryLane {
         });
         static_for<0, Z>([&](auto ic) {
             constexpr int I = decltype(ic)::value;
-            uint64_t Mi[NW];
-            expand_masks<H, NW>(f_hash_c<S>(lmer<I, S>(W)), Mi);
-            sor.template push<I>(Mi);
+            if constexpr (GATHER) {
+                sor.template push<I>(f_hash_c<S>(lmer<I, S>(W)));
+            } else {
+                uint64_t Mi[NW];
+                expand_masks<H, NW>(f_hash_c<S>(lmer<I, S>(W)), Mi);
+                sor.template push<I>(Mi);
+            }
         });
         static_for<0, kLA>([&](auto qc) { this->template look<decltype(qc)::value, decltype(qc)::value == 0>(W, prm, stage); });
     }
@@ -615,11 +731,15 @@ struct QueryLane {
             sh32[4] = hi.x; sh32[5] = hi.y; sh32[6] = hi.z; sh32[7] = hi.w;
         }
 #endif
-        uint64_t Mn[NW];
-        expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
-        const uint64_t shard[4] = {((uint64_t)sh32[1] << 32) | sh32[0], ((uint64_t)sh32[3] << 32) | sh32[2],
-                                   ((uint64_t)sh32[5] << 32) | sh32[4], ((uint64_t)sh32[7] << 32) | sh32[6]};
-        return sor.template push_test<J + Z>(Mn, shard) == 0;
+        if constexpr (GATHER) {
+            return sor.template push_test<J + Z>(f_hash_c<S>(lmer<J + Z, S>(W)), sh32) == 0;
+        } else {
+            uint64_t Mn[NW];
+            expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
+            const uint64_t shard[4] = {((uint64_t)sh32[1] << 32) | sh32[0], ((uint64_t)sh32[3] << 32) | sh32[2],
+                                       ((uint64_t)sh32[5] << 32) | sh32[4], ((uint64_t)sh32[7] << 32) | sh32[6]};
+            return sor.template push_test<J + Z>(Mn, shard) == 0;
+        }
     }
 };
 
