@@ -472,13 +472,15 @@ def run_cuda(args):
         q_runs_g = qk_kmers * (d_runs + 1.0 / per_read) / (qk * 1e-3) / 1e9
         # the best any read-modify-write form reached (1 RED, 4 REDs, one 32-byte TMA reduction) / any load form
         rmw_ceiling = max(x for x in (rs.get("red_or_b64_x4"), rs.get("red_or_b64_x1"), rs.get("tma_reduce_or_32B")) if x)
-        ld_ceiling = max(x for x in (rs.get("ld_nc_256"), rs.get("cp_async_2x16")) if x)
+        ld_ceiling = max(x for x in (rs.get("ld_nc_256"), rs.get("cp_async_2x16"), rs.get("ld_nc_256_L2_64B"),
+                                     rs.get("cp_async_2x16_L2_64B")) if x)
         roof["insert_kernel"]["random_sector"] = {
             "achieved_g_per_s": ins_runs_g, "ceiling_g_per_s": rmw_ceiling, "frac": ins_runs_g / rmw_ceiling,
             "ceiling": "random read-modify-write sectors/s over %d MiB, best of 1 RED, 4 REDs, one TMA reduction" % (num_bits >> 23)}
         roof["query_kernel"]["random_sector"] = {
             "achieved_g_per_s": q_runs_g, "ceiling_g_per_s": ld_ceiling, "frac": q_runs_g / ld_ceiling,
-            "ceiling": "random sector loads/s over %d MiB, best of one 256-bit ld.global.nc and 2 x 16-byte cp.async" % (num_bits >> 23)}
+            "ceiling": "random sector loads/s over %d MiB, best of one 256-bit ld.global.nc and 2 x 16-byte cp.async, "
+                       "each with and without the .L2::64B hint" % (num_bits >> 23)}
         for kk in ("insert_kernel", "query_kernel"):  # which limit binds this kernel: instructions or random sectors
             r = roof[kk]
             busy = dict(r.get("busy_fraction_of_measured_limit", {"alu_pipe": r["frac"]}))
@@ -616,7 +618,8 @@ def measure_ceilings(sbf, filter_bytes, gpu_index, sm_max_mhz):
         per_s[name] = g_per_s
         clocks[name] = mhz
         per_clk[name] = g_per_s * 1e3 / (mhz if mhz else sm_max_mhz)
-    names = ["red_or_b64_x4", "red_or_b64_x1", "ld_nc_256", "cp_async_2x16", "tma_reduce_or_32B"]
+    names = ["red_or_b64_x4", "red_or_b64_x1", "ld_nc_256", "cp_async_2x16", "tma_reduce_or_32B", "ld_nc_256_L2_64B",
+             "cp_async_2x16_L2_64B"]
     rnd = {}
     for mode, nm in enumerate(names):
         try:

@@ -235,7 +235,8 @@ int sbf_get_timing(sbf_t *f, float *ms3);
  * sbf_ceiling_random_sector — random 32-byte-sector accesses per second (in 1e9/s) over a zeroed scratch array of
  *   array_bytes (rounded down to a power of two), allocated and freed inside the call.  mode 0: 4 x red.or.b64 per
  *   sector (the insert kernel's flush), 1: 1 x red.or.b64, 2: one 256-bit ld.global.nc, 3: 2 x 16-byte cp.async into
- *   shared memory (the query kernels' staging), 4: one 32-byte cp.reduce.async.bulk .or.b64 (TMA reduction).
+ *   shared memory, 4: one 32-byte cp.reduce.async.bulk .or.b64 (TMA reduction), 5: mode 2 with the .L2::64B
+ *   prefetch-size hint, 6: mode 3 with the .L2::64B hint (the query kernels' staging, exactly).
  * Both synchronise the device.
  */
 int sbf_ceiling_pipe_modes(void);

@@ -85,12 +85,14 @@ __device__ __forceinline__ uint64_t mix64(uint64_t x)
 //      2: one 256-bit ld.global.nc of a random sector
 //      3: 2 x 16-byte cp.async.cg into shared memory, read back (what the query kernels issue per run)
 //      4: one 32-byte cp.reduce.async.bulk .or.b64 from shared memory (TMA reduction) per random sector
+//      5: mode 2 with the .L2::64B prefetch-size hint (a miss pulls 64 B from DRAM instead of 128 B)
+//      6: mode 3 with the .L2::64B hint (exactly what the query kernels issue per run)
 constexpr int kRandTPB = 128;
 template <int MODE>
 __global__ void __launch_bounds__(kRandTPB) random_sector_kernel(uint64_t *arr, uint64_t sector_mask, uint32_t per_thread, uint64_t *sink)
 {
     constexpr int kSlots = 8; // staged sectors in flight per thread (the query kernels keep up to kLA + 1 = 8)
-    __shared__ __align__(16) uint64_t stage[MODE == 3 ? kSlots : 2][kRandTPB][4];
+    __shared__ __align__(16) uint64_t stage[(MODE == 3 || MODE == 6) ? kSlots : 2][kRandTPB][4];
     const uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     uint64_t acc = 0;
     for (uint32_t i = 0; i < per_thread; ++i) {
@@ -106,6 +108,17 @@ __global__ void __launch_bounds__(kRandTPB) random_sector_kernel(uint64_t *arr, 
             uint64_t w0, w1, w2, w3;
             asm volatile("ld.global.nc.v4.u64 {%0,%1,%2,%3}, [%4];" : "=l"(w0), "=l"(w1), "=l"(w2), "=l"(w3) : "l"(p));
             acc += w0 ^ w1 ^ w2 ^ w3;
+        } else if (MODE == 5) {
+            uint64_t w0, w1, w2, w3;
+            asm volatile("ld.global.nc.L2::64B.v4.u64 {%0,%1,%2,%3}, [%4];" : "=l"(w0), "=l"(w1), "=l"(w2), "=l"(w3) : "l"(p));
+            acc += w0 ^ w1 ^ w2 ^ w3;
+        } else if (MODE == 6) {
+            const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(&stage[i % kSlots][threadIdx.x][0]);
+            asm volatile("cp.async.cg.shared.global.L2::64B [%0], [%1], 16;" ::"r"(s0), "l"(p) : "memory");
+            asm volatile("cp.async.cg.shared.global.L2::64B [%0], [%1], 16;" ::"r"(s0 + 16), "l"(p + 2) : "memory");
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group 7;" ::: "memory");
+            acc += stage[(i + 1) % kSlots][threadIdx.x][0] ^ stage[(i + 1) % kSlots][threadIdx.x][3];
         } else if (MODE == 3) {
             const uint32_t s0 = (uint32_t)__cvta_generic_to_shared(&stage[i % kSlots][threadIdx.x][0]);
             asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s0), "l"(p) : "memory");
@@ -123,7 +136,7 @@ __global__ void __launch_bounds__(kRandTPB) random_sector_kernel(uint64_t *arr, 
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
     }
-    if (MODE == 3) asm volatile("cp.async.wait_group 0;" ::: "memory");
+    if (MODE == 3 || MODE == 6) asm volatile("cp.async.wait_group 0;" ::: "memory");
     if (MODE == 4) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     if (acc == 0x1234567u) sink[0] = acc;
 }
@@ -203,7 +216,7 @@ int sbf_ceiling_pipe_rate(int mode, int iters, double *g_warp_inst_per_s_per_sms
 
 int sbf_ceiling_random_sector(int mode, uint64_t array_bytes, double *g_accesses_per_s)
 {
-    if (mode < 0 || mode > 4 || !g_accesses_per_s || array_bytes < 4096) return SBF_ERR_INVALID_ARG;
+    if (mode < 0 || mode > 6 || !g_accesses_per_s || array_bytes < 4096) return SBF_ERR_INVALID_ARG;
     uint64_t sectors = 1;
     while (sectors * 2 * 32 <= array_bytes) sectors *= 2; // power of two
     int dev = 0, sms = 0;
@@ -229,7 +242,9 @@ int sbf_ceiling_random_sector(int mode, uint64_t array_bytes, double *g_accesses
         case 1: err = launch_rand<1>(arr, sectors - 1, per_thread, sink, blocks); break;
         case 2: err = launch_rand<2>(arr, sectors - 1, per_thread, sink, blocks); break;
         case 3: err = launch_rand<3>(arr, sectors - 1, per_thread, sink, blocks); break;
-        default: err = launch_rand<4>(arr, sectors - 1, per_thread, sink, blocks); break;
+        case 4: err = launch_rand<4>(arr, sectors - 1, per_thread, sink, blocks); break;
+        case 5: err = launch_rand<5>(arr, sectors - 1, per_thread, sink, blocks); break;
+        default: err = launch_rand<6>(arr, sectors - 1, per_thread, sink, blocks); break;
         }
         cudaEventRecord(e1);
         if (err == cudaSuccess) err = cudaEventSynchronize(e1);

@@ -692,9 +692,9 @@ struct QueryLane {
         sb[Q % kNS] = start;
         laPrev = shNew;
     }
-    // k-mer J of the current 16-position block: returns true iff all its H(k-s+1) bits are set in its shard
+    // k-mer J of the current 16-position block: returns 0 iff all its H(k-s+1) bits are set in its shard
     template <int J>
-    __device__ __forceinline__ bool step(const uint32_t (&W)[NWIN], const StreamParams &prm, uint4 *stage)
+    __device__ __forceinline__ uint32_t step(const uint32_t (&W)[NWIN], const StreamParams &prm, uint4 *stage)
     {
         // a6: if a run starts here, its sector was staged kLA positions ago: take it into the shard registers.
 #if SBF_PRED_RELOAD
@@ -732,13 +732,14 @@ struct QueryLane {
         }
 #endif
         if constexpr (GATHER) {
-            return sor.template push_test<J + Z>(f_hash_c<S>(lmer<J + Z, S>(W)), sh32) == 0;
+            return sor.template push_test<J + Z>(f_hash_c<S>(lmer<J + Z, S>(W)), sh32);
         } else {
             uint64_t Mn[NW];
             expand_masks<H, NW>(f_hash_c<S>(lmer<J + Z, S>(W)), Mn);
             const uint64_t shard[4] = {((uint64_t)sh32[1] << 32) | sh32[0], ((uint64_t)sh32[3] << 32) | sh32[2],
                                        ((uint64_t)sh32[5] << 32) | sh32[4], ((uint64_t)sh32[7] << 32) | sh32[6]};
-            return sor.template push_test<J + Z>(Mn, shard) == 0;
+            const uint64_t miss = sor.template push_test<J + Z>(Mn, shard);
+            return (uint32_t)miss | (uint32_t)(miss >> 32);
         }
     }
 };
@@ -876,7 +877,7 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
             uint32_t res16 = 0;
             static_for<0, 16>([&](auto jc) {
                 constexpr int J = decltype(jc)::value;
-                if (ql.template step<J>(W, prm, stage)) res16 |= 1u << J;
+                if (ql.template step<J>(W, prm, stage) == 0) res16 |= 1u << J;
             });
             res16 &= ~v16; // a1: positions without a valid k-mer answer false
 #pragma unroll
@@ -969,12 +970,12 @@ __global__ void __launch_bounds__(kRecTPB, SBF_MINB_R) stream_rec_kernel(const S
         uint32_t res16 = 0;
         static_for<0, 8>([&](auto jc) {
             constexpr int J = decltype(jc)::value;
-            if (ql.template step<J>(W, prm, stage)) res16 |= 1u << J;
+            if (ql.template step<J>(W, prm, stage) == 0) res16 |= 1u << J;
         });
         if (16 * b + 8 < nk)
             static_for<8, 16>([&](auto jc) {
                 constexpr int J = decltype(jc)::value;
-                if (ql.template step<J>(W, prm, stage)) res16 |= 1u << J;
+                if (ql.template step<J>(W, prm, stage) == 0) res16 |= 1u << J;
             });
 #pragma unroll
         for (int i = 0; i + 1 < NWIN; ++i) W[i] = W[i + 1];
