@@ -28,7 +28,7 @@ constexpr int kPipeCTAsPerSM = 4; // 32 warps per SM = 8 per SMSP, all resident 
 template <int MODE>
 __device__ __forceinline__ void pipe_op(uint32_t (&r)[kPipeChains], int c, int u, uint32_t k0, uint32_t k1)
 {
-    // which opcode this slot gets: 0 LOP3, 1 IMAD, 2 SHF, 3 IDP.4A
+    // which opcode this slot gets: 0 LOP3, 1 IMAD, 2 SHF, 3 IDP.4A, 4 IMAD.HI, 5 PRMT
     int op;
     const int slot = u * kPipeChains + c;
     if (MODE == 0) op = 0;
@@ -39,12 +39,18 @@ __device__ __forceinline__ void pipe_op(uint32_t (&r)[kPipeChains], int c, int u
     else if (MODE == 5) op = (slot & 7) == 7 ? 1 : 0;       // 7 : 1
     else if (MODE == 6) op = (slot & 1) ? 2 : 0;            // LOP3 : SHF = 1 : 1 (same pipe)
     else if (MODE == 7) op = 3;
-    else op = (slot & 1) ? 3 : 0;                           // LOP3 : IDP.4A = 1 : 1
+    else if (MODE == 8) op = (slot & 1) ? 3 : 0;            // LOP3 : IDP.4A = 1 : 1
+    else if (MODE == 9) op = 4;
+    else if (MODE == 10) op = (slot & 1) ? 4 : 0;           // LOP3 : IMAD.HI = 1 : 1
+    else if (MODE == 11) op = 5;
+    else op = (slot & 3) == 3 ? 4 : 0;                      // LOP3 : IMAD.HI = 3 : 1
     uint32_t &x = r[c];
     if (op == 0) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(x) : "r"(k0), "r"(k1));
     else if (op == 1) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(x) : "r"(k0), "r"(k1));
     else if (op == 2) asm volatile("shf.r.wrap.b32 %0, %0, %1, %2;" : "+r"(x) : "r"(k0), "r"(k1));
-    else asm volatile("dp4a.u32.u32 %0, %0, %1, %2;" : "+r"(x) : "r"(k0), "r"(k1));
+    else if (op == 3) asm volatile("dp4a.u32.u32 %0, %0, %1, %2;" : "+r"(x) : "r"(k0), "r"(k1));
+    else if (op == 4) asm volatile("mad.hi.u32 %0, %0, %1, %2;" : "+r"(x) : "r"(k0), "r"(k1));
+    else asm volatile("prmt.b32 %0, %0, %1, %2;" : "+r"(x) : "r"(k0), "r"(k1));
 }
 
 template <int MODE>
@@ -71,8 +77,9 @@ __global__ void __launch_bounds__(kPipeTPB) pipe_rate_kernel(uint32_t *sink, int
 }
 
 const char *const kPipeModeName[] = {"LOP3", "IMAD", "SHF", "LOP3:IMAD 1:1", "LOP3:IMAD 3:1", "LOP3:IMAD 7:1",
-                                     "LOP3:SHF 1:1", "IDP.4A", "LOP3:IDP.4A 1:1"};
-constexpr int kPipeModes = 9;
+                                     "LOP3:SHF 1:1", "IDP.4A", "LOP3:IDP.4A 1:1", "IMAD.HI", "LOP3:IMAD.HI 1:1", "PRMT",
+                                     "LOP3:IMAD.HI 3:1"};
+constexpr int kPipeModes = 13;
 
 __device__ __forceinline__ uint64_t mix64(uint64_t x)
 {
@@ -189,7 +196,11 @@ int sbf_ceiling_pipe_rate(int mode, int iters, double *g_warp_inst_per_s_per_sms
         case 5: err = launch_pipe<5>(sink, iters, cyc, blocks); break;
         case 6: err = launch_pipe<6>(sink, iters, cyc, blocks); break;
         case 7: err = launch_pipe<7>(sink, iters, cyc, blocks); break;
-        default: err = launch_pipe<8>(sink, iters, cyc, blocks); break;
+        case 8: err = launch_pipe<8>(sink, iters, cyc, blocks); break;
+        case 9: err = launch_pipe<9>(sink, iters, cyc, blocks); break;
+        case 10: err = launch_pipe<10>(sink, iters, cyc, blocks); break;
+        case 11: err = launch_pipe<11>(sink, iters, cyc, blocks); break;
+        default: err = launch_pipe<12>(sink, iters, cyc, blocks); break;
         }
         cudaEventRecord(e1);
         if (err == cudaSuccess) err = cudaEventSynchronize(e1);

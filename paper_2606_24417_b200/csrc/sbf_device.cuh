@@ -47,6 +47,9 @@
 #ifndef SBF_GATHER
 #define SBF_GATHER 1 // query: byte-gather sliding test (SlidingGather) instead of 256-bit masks where it applies (H <= 4, k-s+1 in {1,2,4,8})
 #endif
+#ifndef SBF_GATHER_PAIRED
+#define SBF_GATHER_PAIRED 1 // SlidingGather, H = 4: the selectors of words q, q+1 share a register (one shift + one insert for both)
+#endif
 #ifndef SBF_GATHER_FMA_SHIFT
 #define SBF_GATHER_FMA_SHIFT 0 // SlidingGather: right shifts of the y fields as multiply-high (fma pipe)
 #endif
@@ -486,6 +489,7 @@ template <int WO, int H>
 struct SlidingGather {
     static_assert(H >= 1 && H <= 4 && (WO == 1 || WO == 2 || WO == 4 || WO == 8), "gather form: H <= 4, k-s+1 in {1,2,4,8}");
     static constexpr int NW = H, Wd = 64 / H, NSET = WO > 4 ? 2 : 1;
+    static constexpr bool PAIRED = SBF_GATHER_PAIRED != 0 && H == 4;
     uint32_t S[NSET][NW], T[NSET][NW];
     __device__ __forceinline__ void clear()
     {
@@ -536,12 +540,34 @@ struct SlidingGather {
         static_for<0, NW>([&](auto qc) {
             constexpr int q = decltype(qc)::value, off = q * Wd;
             static_assert(off % 32 + 6 <= 32, "a 6-bit slice straddles the halves of the hash");
-            constexpr uint32_t nib = 7u << (4 * rr);
-            const uint32_t y = shift_to<off % 32 + 3 - 4 * rr>(off < 32 ? lo : hi); // y field moved to nibble rr, junk around it
-            S[a][q] = bitsel(y, S[a][q], nib);
+            if constexpr (PAIRED) {
+                // H = 4: the fields of words q and q+1 sit 16 bits apart in one half of the hash, so ONE shift and ONE
+                // masked insert serve both: S[q] keeps word q's selector in its low half and word q+1's in its high half
+                if constexpr ((q & 1) == 0) {
+                    constexpr uint32_t nib2 = 0x00070007u << (4 * rr);
+                    S[a][q] = bitsel(shift_to<3 - 4 * rr>(q < 2 ? lo : hi), S[a][q], nib2);
+                }
+            } else {
+                constexpr uint32_t nib = 7u << (4 * rr);
+                const uint32_t y = shift_to<off % 32 + 3 - 4 * rr>(off < 32 ? lo : hi); // y field moved to nibble rr, junk around it
+                S[a][q] = bitsel(y, S[a][q], nib);
+            }
             constexpr uint32_t keep = 0x3210u & ~(0xFu << (4 * rr)); // T[q] bytes stay, byte rr <- onehot byte q
             T[a][q] = prmt(T[a][q], onehot, keep | ((uint32_t)(4 + q) << (4 * rr)));
         });
+    }
+    __device__ __forceinline__ uint32_t selector(int a, int q) const
+    {
+        if constexpr (PAIRED) {
+            if (q & 1) {
+#if SBF_GATHER_FMA_SHIFT
+                return __umulhi(S[a][q - 1], 1u << 16);
+#else
+                return S[a][q - 1] >> 16;
+#endif
+            }
+        }
+        return S[a][q];
     }
     // bits of the k-mer's H * WO positions that are NOT set in the shard (0 = present); sh32 = the sector as 8 halves
     template <int E>
@@ -552,7 +578,7 @@ struct SlidingGather {
 #pragma unroll
         for (int a = 0; a < NSET; ++a)
 #pragma unroll
-            for (int q = 0; q < NW; ++q) miss |= T[a][q] & ~prmt(sh32[2 * q], sh32[2 * q + 1], S[a][q]);
+            for (int q = 0; q < NW; ++q) miss |= T[a][q] & ~prmt(sh32[2 * q], sh32[2 * q + 1], selector(a, q));
         return miss;
     }
 };

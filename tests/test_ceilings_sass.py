@@ -17,6 +17,7 @@ EXPECT = {
     0: {"LOP3": 256}, 1: {"IMAD": 256}, 2: {"SHF": 256},
     3: {"LOP3": 128, "IMAD": 128}, 4: {"LOP3": 192, "IMAD": 64}, 5: {"LOP3": 224, "IMAD": 32},
     6: {"LOP3": 128, "SHF": 128}, 7: {"IDP": 256}, 8: {"LOP3": 128, "IDP": 128},
+    9: {"IMAD": 256}, 10: {"LOP3": 128, "IMAD": 128}, 11: {"PRMT": 256}, 12: {"LOP3": 192, "IMAD": 64},
 }
 
 
