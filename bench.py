@@ -35,9 +35,14 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "G k-mers/s insert+query (1 step = insert the sequence + query one read batch)"
-# ALGORITHMIC integer instructions per valid k-mer (defaults k=31 m=16 s=28 H=4), split by the
-# pipe they issue on: the multiplies of g, sigma and f (1 + 3 + 3 IMAD-class) go to the fma pipe, the rest to the alu pipe.
-OPS_PER_KMER = {"insert": {"alu": 63.0, "fma": 7.0}, "query": {"alu": 56.0, "fma": 7.0}}
+# ALGORITHMIC integer instructions per valid k-mer of the fused kernels (defaults k=31 m=16 s=28 H=4), derived part by part in
+# DESIGN.md §6, split by how they issue: "alu" (LOP3/SHF/PRMT/VIMNMX/ISETP class), "fma" (32-bit IMAD / IDP.4A: the
+# fma pipe at full rate), "wide" (IMAD.WIDE / IMAD.HI, the 64-bit-result multiplies of sigma, f, the sector address
+# and the selector packing: half rate and, measured, not overlapping the alu pipe).  SURVEY.md §8(d)'s planning figures
+# were 70 (insert) and 63 (query); the query's byte-gather formulation of round 2 needs fewer (the survey's 26 for the bit
+# tests became 21), so it is restated here — quoting the kernel against the survey's 63 would give a fraction above 1.
+OPS_PER_KMER = {"insert": {"alu": 63.0, "fma": 5.0, "wide": 2.0}, "query": {"alu": 39.0, "fma": 4.0, "wide": 4.0}}
+SURVEY_OPS_PER_KMER = {"insert": 70.0, "query": 63.0}
 N_SMSP = 148 * 4
 # What the kernels EXECUTE (warp instructions per launch, by pipe): ncu counters of a committed capture, static.
 PIPES_CSV = os.path.join("profiles", "pipes_r02.csv")
@@ -451,8 +456,10 @@ def run_cuda(args):
         clock_mhz = sm_max_mhz                       # rooflines are quoted at the maximum SM clock
         ex_i, ex_i_src = load_pipes("insert_kernel")
         ex_q, ex_q_src = load_pipes("query_kernel")
-        roof = {"insert_kernel": alu_roofline(OPS_PER_KMER["insert"], n_ins_kmers, ik, ceilings, clock_mhz, ex_i),
-                "query_kernel": alu_roofline(OPS_PER_KMER["query"], qk_kmers, qk, ceilings, clock_mhz, ex_q),
+        roof = {"insert_kernel": alu_roofline(OPS_PER_KMER["insert"], n_ins_kmers, ik, ceilings, clock_mhz, ex_i,
+                                              SURVEY_OPS_PER_KMER["insert"]),
+                "query_kernel": alu_roofline(OPS_PER_KMER["query"], qk_kmers, qk, ceilings, clock_mhz, ex_q,
+                                             SURVEY_OPS_PER_KMER["query"]),
                 "pack_kernel_ms_mean": statistics.mean(pack_ms), "count_kernel_ms_mean": statistics.mean(count_ms)}
         roof["insert_kernel"]["executed_source"], roof["query_kernel"]["executed_source"] = ex_i_src, ex_q_src
         # HBM: algorithmic bytes of the fused kernels (packed 2-bit words + mask + one sector read/write per run)
@@ -634,23 +641,30 @@ def measure_ceilings(sbf, filter_bytes, gpu_index, sm_max_mhz):
             "random_sector_g_per_s": rnd, "random_sector_array_bytes": int(min(filter_bytes, 8 << 30))}
 
 
-def alu_roofline(ops, n_units, ms, ceil, clock_mhz, executed):
+def alu_roofline(ops, n_units, ms, ceil, clock_mhz, executed, survey_ops=None):
     """Instruction roofline of one kernel.  achieved = ALGORITHMIC lane-ops per second.  peak = the rate the SM
-    sub-partitions can issue that algorithmic mix at: per unit the alu-pipe ops need ops_alu / r_alu clocks, the
-    fma-pipe ops ops_fma / r_fma, and all of them together (ops_alu + ops_fma) / r_issue; the slowest binds
-    (r_* measured: pure LOP3, pure IMAD, LOP3:IMAD 1:1).  `executed` (ncu) gives the same three times for the
-    instructions the kernel really issues: their ratio to the kernel's duration is how busy each limit is."""
+    sub-partitions can issue that algorithmic mix at, from rates measured in this run: per warp of 32 units the
+    alu-pipe ops need ops_alu / r_alu clocks PLUS c_wide clocks per wide multiply (the LOP3:IMAD.HI mixes show the
+    64-bit-result multiplies serialise with the alu pipe: c_wide = 4 / rate(LOP3:IMAD.HI 3:1) - 3 / r_alu), the
+    fma-pipe ops (ops_fma + ops_wide) / r_fma, and all of them together total / r_issue; the slowest binds.
+    `executed` (ncu) gives how busy the instructions the kernel really issues keep each of those limits."""
     pr = ceil["pipe_warp_inst_per_clk_per_smsp"]
     r_alu, r_fma, r_issue = pr["LOP3"], pr["IMAD"], pr["LOP3:IMAD 1:1"]
-    total = ops["alu"] + ops["fma"]
-    clk_per_unit = max(ops["alu"] / r_alu, ops["fma"] / r_fma, total / r_issue)   # per warp of 32 units, per SMSP
+    c_wide = 4.0 / pr["LOP3:IMAD.HI 3:1"] - 3.0 / r_alu if pr.get("LOP3:IMAD.HI 3:1") else 1.0 / r_fma
+    wide = ops.get("wide", 0.0)
+    total = ops["alu"] + ops["fma"] + wide
+    clk_per_unit = max(ops["alu"] / r_alu + wide * c_wide, (ops["fma"] + wide) / r_fma, total / r_issue)  # per warp, per SMSP
     lanes_per_s = 32.0 * N_SMSP * clock_mhz * 1e6
     peak = total / clk_per_unit * lanes_per_s / 1e12                                # T lane-ops/s for this mix
     achieved = total * n_units / (ms * 1e-3) / 1e12
     out = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tiop/s", "frac": achieved / peak, "ms": ms,
            "gkmers_s": n_units / ms / 1e6,
            "algorithmic_ops_per_kmer": dict(ops), "peak_source": "measured: pipe rates alu %.3f fma %.3f issue %.3f "
-           "warp-inst/clk/SMSP x %d SMSP x %.0f MHz" % (r_alu, r_fma, r_issue, N_SMSP, clock_mhz)}
+           "warp-inst/clk/SMSP, %.2f clk per wide multiply next to alu work, x %d SMSP x %.0f MHz"
+           % (r_alu, r_fma, r_issue, c_wide, N_SMSP, clock_mhz)}
+    if survey_ops:
+        out["survey_planning_ops_per_kmer"] = survey_ops
+        out["frac_with_survey_count"] = survey_ops * n_units / (ms * 1e-3) / 1e12 / (lanes_per_s * r_alu / 1e12)
     if executed:
         cyc = ms * 1e-3 * clock_mhz * 1e6 * N_SMSP                                   # SMSP-cycles of the launch
         busy = {"alu_pipe": executed["inst_alu"] / r_alu / cyc, "fma_pipe": executed["inst_fma"] / r_fma / cyc,

@@ -200,6 +200,22 @@ __device__ __forceinline__ uint32_t pack4(uint32_t v, uint32_t &inv4)
     return __dp4a(c, 0x01041040u, 0u);
 }
 
+// The same codes with the validity test deferred: returns TWICE the 8 code bits (bit 0 is zero) and ORs into `bad` the
+// XOR of the four symbols (case bit cleared) with the letters of their own codes — zero iff all four are ACGT.  Almost
+// every thread sees only valid symbols, so the per-symbol invalid flags (pack4) are only worked out when `bad` is not zero.
+//   per byte t = 2 * code: bit 2 = b2, bit 1 = b1 ^ b2 (three instructions for four symbols); t indexes an 8-entry
+//   byte table "A.C.G.T." directly (no shift), and the byte dot product gathers 2 * (c0 c1 c2 c3).
+__device__ __forceinline__ uint32_t pack4_codes2(uint32_t v, uint32_t &bad)
+{
+    const uint32_t u = v & 0x06060606u;
+    const uint32_t t = (u ^ (u >> 1)) & 0x06060606u;
+    const uint32_t sel = __dp4a(t, 0x00001001u, 0u) + (__dp4a(t, 0x10010000u, 0u) << 8); // the four 2 * codes as nibbles
+    uint32_t letters;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(letters) : "r"(0x00430041u), "r"(0x00540047u), "r"(sel));
+    bad |= (v & 0xDFDFDFDFu) ^ letters;
+    return __dp4a(t, 0x01041040u, 0u);
+}
+
 #ifdef SBF_DEFINE_AUX_KERNELS // non-template kernels: defined in one translation unit (sbf_api.cu)
 // 32 symbols starting at b0 as eight little-endian 4-byte groups ('N' past the end)
 __device__ __forceinline__ void load32(const uint8_t *__restrict__ seq, uint64_t b0, uint64_t len, int aligned16, uint32_t (&v)[8])
@@ -238,13 +254,19 @@ __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ s
     if (i == 0 && flag_zero != nullptr) *flag_zero = 0;
     uint32_t v[8];
     load32(seq, b0, len, aligned16, v);
-    uint32_t word[2] = {0, 0}, inv = 0;
+    uint32_t word[2] = {0, 0}, inv = 0, bad = 0;
 #pragma unroll
     for (int w = 0; w < 8; ++w) {
-        uint32_t i4;
-        const uint32_t c8 = pack4(v[w], i4);
-        word[w >> 2] |= c8 << (24 - 8 * (w & 3));
-        inv |= i4 << (4 * w);
+        const uint32_t c9 = pack4_codes2(v[w], bad); // 2 * (8 code bits)
+        word[w >> 2] |= (w & 3) == 3 ? c9 >> 1 : c9 << (23 - 8 * (w & 3));
+    }
+    if (bad != 0) { // some symbol of these 32 is not ACGT (or lies past the end): which ones
+#pragma unroll
+        for (int w = 0; w < 8; ++w) {
+            uint32_t i4;
+            (void)pack4(v[w], i4);
+            inv |= i4 << (4 * w);
+        }
     }
     // B of the next 32 (k > 33: 64) symbols: the following threads' words through shared memory; only the last thread(s)
     // of the CTA classify them themselves (a per-warp exchange would send one lane in 32 down that divergent path)

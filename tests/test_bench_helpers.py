@@ -64,6 +64,12 @@ def test_instruction_roofline_model():
     # an fma-heavy mix is bound by issue, not by either pipe
     r = bench.alu_roofline({"alu": 30.0, "fma": 30.0}, n, ms, ceil, 1000.0, None)
     assert abs(r["peak"] - 1.0 * 32 * 592 * 1e9 / 1e12) < 1e-9
+    # wide multiplies (IMAD.WIDE / IMAD.HI) add their measured cost to the alu-pipe time: LOP3:IMAD.HI 3:1 at 4/9 per clock
+    # means 3 LOP3 (6 clocks) + 1 IMAD.HI take 9 clocks, i.e. 3 clocks per wide multiply
+    ceil["pipe_warp_inst_per_clk_per_smsp"]["LOP3:IMAD.HI 3:1"] = 4.0 / 9.0
+    r = bench.alu_roofline({"alu": 40.0, "fma": 4.0, "wide": 4.0}, n, ms, ceil, 1000.0, None, survey_ops=63.0)
+    assert abs(r["peak"] - 48.0 / (80.0 + 12.0) * 32 * 592 * 1e9 / 1e12) < 1e-6
+    assert abs(r["frac_with_survey_count"] - 63.0 * n / 1e-3 / (32 * 592 * 1e9 * 0.5)) < 1e-9
 
 
 def test_static_profile_tables_load():
