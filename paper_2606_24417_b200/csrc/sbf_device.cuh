@@ -47,6 +47,9 @@
 #ifndef SBF_GATHER
 #define SBF_GATHER 1 // query: byte-gather sliding test (SlidingGather) instead of 256-bit masks where it applies (H <= 4, k-s+1 in {1,2,4,8})
 #endif
+#ifndef SBF_MIN3_ASM
+#define SBF_MIN3_ASM 1 // sliding minimum: three-input minima as opaque asm (kept as VIMNMX3 instead of being re-associated)
+#endif
 #ifndef SBF_GATHER_PAIRED
 #define SBF_GATHER_PAIRED 1 // SlidingGather, H = 4: the selectors of words q, q+1 share a register (one shift + one insert for both)
 #endif
@@ -387,7 +390,18 @@ __device__ __forceinline__ uint64_t lmer(const uint32_t (&W)[NWIN])
     }
 }
 
-__device__ __forceinline__ uint32_t min3u(uint32_t a, uint32_t b, uint32_t c) { return min(min(a, b), c); }
+// three-input minimum as an opaque pair of min.u32 (ptxas fuses it into one VIMNMX3); written with min(min(a, b), c)
+// the optimiser re-associates the sliding-minimum tree across positions into two-input minima — about twice as many
+__device__ __forceinline__ uint32_t min3u(uint32_t a, uint32_t b, uint32_t c)
+{
+#if SBF_MIN3_ASM
+    uint32_t r;
+    asm("{\n\t.reg .u32 t;\n\tmin.u32 t, %1, %2;\n\tmin.u32 %0, t, %3;\n\t}" : "=r"(r) : "r"(a), "r"(b), "r"(c));
+    return r;
+#else
+    return min(min(a, b), c);
+#endif
+}
 
 // Sliding minimum of the last WN keys, streaming: keys arrive one per step, E = step phase (mod 16
 // is all that matters).  Levels c3 = min of the last 3, c9 = min of the last 9; the window of WN is
