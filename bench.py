@@ -37,11 +37,11 @@ if ROOT not in sys.path:
 METRIC = "G k-mers/s insert+query (1 step = insert the sequence + query one read batch)"
 # ALGORITHMIC integer instructions per valid k-mer of the fused kernels (defaults k=31 m=16 s=28 H=4), derived part by part in
 # DESIGN.md §6, split by how they issue: "alu" (LOP3/SHF/PRMT/VIMNMX/ISETP class), "fma" (32-bit IMAD / IDP.4A: the
-# fma pipe at full rate), "wide" (IMAD.WIDE / IMAD.HI, the 64-bit-result multiplies of sigma, f, the sector address
-# and the selector packing: half rate and, measured, not overlapping the alu pipe).  SURVEY.md §8(d)'s planning figures
+# fma pipe at full rate), "wide" (IMAD.WIDE / IMAD.HI, the 64-bit-result multiplies of sigma, f and the sector
+# address: half rate and, measured, not overlapping the alu pipe).  SURVEY.md §8(d)'s planning figures
 # were 70 (insert) and 63 (query); the query's byte-gather formulation of round 2 needs fewer (the survey's 26 for the bit
 # tests became 21), so it is restated here — quoting the kernel against the survey's 63 would give a fraction above 1.
-OPS_PER_KMER = {"insert": {"alu": 63.0, "fma": 5.0, "wide": 2.0}, "query": {"alu": 39.0, "fma": 4.0, "wide": 4.0}}
+OPS_PER_KMER = {"insert": {"alu": 63.0, "fma": 5.0, "wide": 2.0}, "query": {"alu": 39.0, "fma": 4.0, "wide": 3.0}}
 SURVEY_OPS_PER_KMER = {"insert": 70.0, "query": 63.0}
 N_SMSP = 148 * 4
 # What the kernels EXECUTE (warp instructions per launch, by pipe): ncu counters of a committed capture, static.
@@ -667,8 +667,9 @@ def alu_roofline(ops, n_units, ms, ceil, clock_mhz, executed, survey_ops=None):
         out["frac_with_survey_count"] = survey_ops * n_units / (ms * 1e-3) / 1e12 / (lanes_per_s * r_alu / 1e12)
     if executed:
         cyc = ms * 1e-3 * clock_mhz * 1e6 * N_SMSP                                   # SMSP-cycles of the launch
-        busy = {"alu_pipe": executed["inst_alu"] / r_alu / cyc, "fma_pipe": executed["inst_fma"] / r_fma / cyc,
-                "issue": executed["inst_total"] / r_issue / cyc}
+        scale = n_units / executed["units"]        # the capture's counts, scaled to this launch's number of k-mers
+        busy = {"alu_pipe": executed["inst_alu"] * scale / r_alu / cyc, "fma_pipe": executed["inst_fma"] * scale / r_fma / cyc,
+                "issue": executed["inst_total"] * scale / r_issue / cyc}
         out["executed_warp_inst_per_kmer"] = {k[5:]: v * 32.0 / executed["units"] for k, v in executed.items()
                                               if k.startswith("inst_")}
         out["busy_fraction_of_measured_limit"] = busy
