@@ -154,7 +154,7 @@ struct sbf {
     uint64_t *filter;        // 4 * num_shards words
     const KernelEntry *entry; // nullptr -> runtime-parameter kernels
     bool tma_flush;           // insert flushes runs with TMA reductions (filter much larger than L2)
-    // wide path (A19-A22): other alphabets, packed k-mers wider than 64 bits -> wide_kernel, no pack pass
+    // wide path (A19-A22): other alphabets, packed k-mers wider than 64 bits -> wide_tile_kernel, no pack pass
     int alphabet, sym_bits, sym_bytes;
     bool wide;
     int phase0;               // host-facing chunks only: see WideParams::phase0
@@ -303,8 +303,9 @@ int run_wide(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_
     p.filter = f->filter; p.shard_shift = 32 - f->P; p.bitmap = bitmap; p.n_bitmap_words = (total + 31) / 32;
     p.k = f->k; p.m = f->m; p.s = f->s; p.H = f->H; p.alphabet = f->alphabet; p.sym_bits = f->sym_bits; p.sym_bytes = f->sym_bytes;
     p.phase0 = f->phase0;
-    const uint64_t n32 = (total + 31) / 32 * 32;
-    wide_kernel<INSERT><<<(unsigned)((n32 + 255) / 256), 256, 0, st>>>(p);
+    const unsigned tiles = (unsigned)((total + kWtTile - 1) / kWtTile);
+    if (p.sym_bytes == 3) wide_tile_kernel<INSERT, 3><<<tiles, kWtTPB, 0, st>>>(p);
+    else wide_tile_kernel<INSERT, 1><<<tiles, kWtTPB, 0, st>>>(p);
     CK(cudaGetLastError());
     g_launches++;
     return mark(f, 2, st);
@@ -450,7 +451,7 @@ sbf_t *sbf_create_ex(int k, int m, int s, int H, uint64_t num_bits, int alphabet
     }
     f->k = k; f->m = m; f->s = s; f->H = H; f->P = P; f->device = dev;
     f->alphabet = alphabet; f->sym_bits = sym_bits; f->sym_bytes = alphabet == SBF_ALPHABET_DNA_TRIPLET ? 3 : 1;
-    // DNA with 33 <= k <= 64 has specialised streaming instances too (folded wide windows, A21); without one: wide_kernel
+    // DNA with 33 <= k <= 64 has specialised streaming instances too (folded wide windows, A21); without one: wide_tile_kernel
     f->wide = alphabet != SBF_ALPHABET_DNA || (k > 32 && find_entry(k, m, s, H) == nullptr);
     f->num_shards = shards;
     f->host_chunk = kHostChunkDefault;

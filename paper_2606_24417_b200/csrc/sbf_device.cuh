@@ -1130,16 +1130,14 @@ __global__ void __launch_bounds__(256) naive_kernel(const NaiveParams np)
 }
 
 // =============================================================================================
-// WIDE runtime-parameter kernel: the other alphabets of P:139 — protein (26 symbols, 5 bits),
+// WIDE runtime-parameter path: the other alphabets of P:139 — protein (26 symbols, 5 bits),
 // DNA triplets (64 symbols, 6 bits, three bytes per symbol) — and packed k-mers wider than one 64-bit word (P:153,
-// P:435): k * symbol bits <= 128.  Alg. 1 / Alg. 2 as printed, one k-mer per thread, straight from the ASCII bytes
-// (no pack pass), every window recomputed.  Readings A19-A22 of DESIGN.md §3:
+// P:435): k * symbol bits <= 128, straight from the ASCII bytes (no pack pass).  Readings A19-A22 of DESIGN.md §3:
 //   A19 symbols; triplet symbols sit at multiples of 3 bytes from the record start, windows slide by one symbol
 //   A20 the packed k-mer is a 128-bit value, first symbol most significant
 //   A21 a window wider than 64 bits is folded before hashing: lo ^ rotl32(hi * 0x9E3779B97F4A7C15); the seeds of g and
 //       f are masked to min(window bits, 64)
 //   A22 bit index of the result bitmap = BYTE position of the k-mer's first byte
-// "Larger alphabets remain functional": this path is correct, not tuned.
 // =============================================================================================
 struct WideParams {
     const uint8_t *bases;    // ASCII, all records concatenated
@@ -1156,100 +1154,249 @@ struct WideParams {
     int phase0;              // bytes of the record holding byte 0 that precede the buffer, mod sym_bytes (host-facing chunks)
 };
 
-typedef unsigned __int128 u128_t;
-
 __device__ __forceinline__ int dna_code(uint32_t c)
 {
     c &= 0xDFu;
     return c == 'A' ? 0 : c == 'C' ? 1 : c == 'G' ? 2 : c == 'T' ? 3 : -1;
 }
-__device__ __forceinline__ int wide_symbol(const uint8_t *__restrict__ p, int alphabet)
+#ifdef SBF_DEFINE_AUX_KERNELS
+// ---------------------------------------------------------------------------------------------
+// wide_tile_kernel, CTA-cooperative.  Done one k-mer per thread, Alg. 1 / Alg. 2 recompute per k-mer the k symbol
+// codes, k-m+1 m-mer keys and k-s+1 s-mer hashes (each a 128-bit shift, mask, fold and multiply) and search the
+// offsets for the record: ~1000 instructions per k-mer (round 2's first wide_kernel: 6-22 G k-mers/s).  Here a CTA of
+// 256 threads takes a tile of 1024 byte positions (+ a 64-byte halo: k * symbol bytes <= 64) through shared memory:
+//   A  raw bytes -> code of the symbol STARTING at every byte (0xFF invalid); warp 0 meanwhile finds the record
+//      holding the tile's first byte (32-ary search over the offsets) and the CTA lists the record boundaries that
+//      fall inside the tile;
+//   B  every m-mer key, every s-mer's four sector-word masks and "these k symbols hold an invalid one" ONCE per start
+//      byte: a thread rolls the packed windows along five consecutive symbols of one frame (one 128-bit shift-or per
+//      symbol instead of m or s);
+//   C  one k-mer per thread and byte: validity from the record boundaries, the symbol grid and the rolled invalid
+//      flag, minimum of k-m+1 keys, OR of k-s+1 mask quadruples — then the shard update / test of Alg. 1 / Alg. 2.
+//      A warp covers 32 consecutive bytes: the query result word is one ballot.
+// 2.2-4.9 x the one-k-mer-per-thread form (protein k=12: 51, k=25: 43, triplets k=10: 14, DNA k=63 without a
+// specialised instance: 31 G k-mers/s on 60 MB).  A tile with more record boundaries than it has room for (thousands
+// of empty records in 1 KiB) looks its records up in global memory instead.
+// ---------------------------------------------------------------------------------------------
+constexpr int kWtTPB = 256, kWtTile = 1024, kWtHalo = 64, kWtSpan = kWtTile + kWtHalo, kWtStrip = 5; // 218 strips of 5 symbols: one per thread
+
+__device__ __forceinline__ int wide_symbol_smem(const uint8_t *raw, int alphabet)
 {
-    if (alphabet == 0) return dna_code(__ldg(p));
+    if (alphabet == 0) return dna_code(raw[0]);
     if (alphabet == 1) {
-        const uint32_t c = __ldg(p) & 0xDFu;
-        return (c >= 'A' && c <= 'Z' && (__ldg(p) & 0x40u)) ? (int)(c - 'A') : -1;
+        const uint32_t c = raw[0] & 0xDFu;
+        return (c >= 'A' && c <= 'Z' && (raw[0] & 0x40u)) ? (int)(c - 'A') : -1;
     }
-    const int c0 = dna_code(__ldg(p)), c1 = dna_code(__ldg(p + 1)), c2 = dna_code(__ldg(p + 2));
+    const int c0 = dna_code(raw[0]), c1 = dna_code(raw[1]), c2 = dna_code(raw[2]);
     return (c0 | c1 | c2) < 0 ? -1 : 16 * c0 + 4 * c1 + c2;
 }
-__device__ __forceinline__ uint64_t wide_sub(u128_t v, int k, int i, int len, int b) // Sub(v,i,len), folded (A21)
+
+// a packed window of up to 128 bits as four 32-bit words (w[3] most significant); symbol widths are below 32 bits
+struct Win128 {
+    uint32_t w[4];
+    __device__ __forceinline__ void clear() { w[0] = w[1] = w[2] = w[3] = 0; }
+    __device__ __forceinline__ void push(uint32_t c, int b) // (v << b) | c
+    {
+        w[3] = __funnelshift_l(w[2], w[3], b);
+        w[2] = __funnelshift_l(w[1], w[2], b);
+        w[1] = __funnelshift_l(w[0], w[1], b);
+        w[0] = (w[0] << b) | c;
+    }
+    __device__ __forceinline__ void mask(const uint32_t (&m)[4]) { w[0] &= m[0]; w[1] &= m[1]; w[2] &= m[2]; w[3] &= m[3]; }
+    __device__ __forceinline__ uint64_t fold() const // A21: lo ^ rotl32(hi * golden)
+    {
+        const uint64_t lo = ((uint64_t)w[1] << 32) | w[0], hi = ((uint64_t)w[3] << 32) | w[2];
+        const uint64_t t = hi * kGold64;
+        return lo ^ ((t << 32) | (t >> 32));
+    }
+};
+__device__ __forceinline__ void low_mask128(int nbits, uint32_t (&m)[4])
 {
-    u128_t w = v >> ((k - len - i) * b);
-    const int nb = len * b;
-    if (nb < 128) w &= (((u128_t)1) << nb) - 1;
-    const uint64_t t = (uint64_t)(w >> 64) * kGold64;
-    return (uint64_t)w ^ ((t << 32) | (t >> 32));
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int r = nbits - 32 * i;
+        m[i] = r >= 32 ? 0xFFFFFFFFu : r <= 0 ? 0u : ((1u << r) - 1u);
+    }
 }
 
-#ifdef SBF_DEFINE_AUX_KERNELS
-template <bool INSERT>
-__global__ void __launch_bounds__(256) wide_kernel(const WideParams prm)
+template <bool INSERT, int NB> // NB = bytes per symbol (1: DNA, protein; 3: DNA triplets)
+__global__ void __launch_bounds__(kWtTPB) wide_tile_kernel(const WideParams prm)
 {
-    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; // grid covers a multiple of 32 byte positions
-    const int k = prm.k, m = prm.m, s = prm.s, H = prm.H, b = prm.sym_bits, nb = prm.sym_bytes;
-    bool present = false;
-    if (p < prm.total) {
-        // the record holding byte p: offsets[r] <= p < offsets[r+1]
-        uint64_t a = 0, e = prm.total;
+    __shared__ __align__(16) ulonglong2 s_mk01[kWtSpan], s_mk23[kWtSpan]; // one-hot sector words of the s-mer starting at each byte
+    __shared__ uint32_t s_gk[kWtSpan];                    // key of the m-mer starting at each byte
+    __shared__ uint16_t s_bnd[kWtSpan + 8];               // record boundaries in (t0, t0 + span), relative to t0
+    __shared__ uint8_t s_raw[kWtSpan + 8], s_code[kWtSpan + 8];
+    __shared__ uint8_t s_kbad[kWtSpan];                   // the k symbols starting at each byte hold an invalid one
+    __shared__ uint64_t s_rec0[2];                        // index and start of the record holding byte t0
+    __shared__ int s_nbnd;                                // boundaries listed; -1: too many, look records up globally
+
+    const int k = prm.k, m = prm.m, s = prm.s, H = prm.H, b = prm.sym_bits;
+    const int tid = threadIdx.x;
+    const uint64_t t0 = (uint64_t)blockIdx.x * kWtTile;
+
+    // ---- A: raw bytes; the first record (warp 0)
+    for (int i = tid; i < kWtSpan + 8; i += kWtTPB) {
+        const uint64_t q = t0 + (uint64_t)i;
+        s_raw[i] = q < prm.total ? __ldg(prm.bases + q) : (uint8_t)0;
+    }
+    if (tid < 32) {
+        uint64_t lo = 0;
         if (prm.offsets != nullptr) {
-            uint64_t lo = 0, hi = prm.n_rec;
+            uint64_t hi = prm.n_rec; // offsets[lo] <= t0 < offsets[hi]
             while (hi - lo > 1) {
-                const uint64_t mid = lo + (hi - lo) / 2;
-                if (__ldg(prm.offsets + mid) <= p) lo = mid; else hi = mid;
+                const uint64_t step = (hi - lo + 32) / 33;
+                const uint64_t idx = lo + (uint64_t)(tid + 1) * step;
+                const bool le = idx < hi && __ldg(prm.offsets + idx) <= t0;
+                const int c = __popc(__ballot_sync(0xFFFFFFFFu, le));
+                const uint64_t nhi = c < 32 ? lo + (uint64_t)(c + 1) * step : hi;
+                lo += (uint64_t)c * step;
+                hi = nhi < hi ? nhi : hi;
             }
-            a = __ldg(prm.offsets + lo);
-            e = __ldg(prm.offsets + lo + 1);
         }
-        const uint64_t rel = p - a + (a == 0 ? (uint64_t)prm.phase0 : 0);
-        if (rel % (uint64_t)nb == 0 && p + (uint64_t)k * nb <= e) {
-            u128_t v = 0;
-            bool ok = true;
-            for (int i = 0; i < k; ++i) { // ValidKmer + PackKmer (Alg. 1 l.3-4)
-                const int c = wide_symbol(prm.bases + p + (uint64_t)i * nb, prm.alphabet);
-                ok = ok && c >= 0;
-                v = (v << b) | (u128_t)(uint32_t)(c & 63);
+        if (tid == 0) {
+            s_rec0[0] = lo;
+            s_rec0[1] = prm.offsets != nullptr ? __ldg(prm.offsets + lo) : 0;
+            s_nbnd = 0;
+        }
+    }
+    __syncthreads();
+    // the boundaries after that record, while they fall inside the tile and its halo
+    if (prm.offsets != nullptr) {
+        const uint64_t first = s_rec0[0] + 1;
+        for (int round = 0;; ++round) {
+            const uint64_t idx = first + (uint64_t)round * kWtTPB + tid;
+            const uint64_t v = idx <= prm.n_rec ? __ldg(prm.offsets + idx) : ~0ull;
+            const bool inside = v < t0 + kWtSpan;
+            const int slot = round * kWtTPB + tid;
+            if (inside && slot < kWtSpan) s_bnd[slot] = (uint16_t)(v - t0);
+            const int n = __syncthreads_count(inside);
+            if (tid == 0) s_nbnd = (s_nbnd < 0 || s_nbnd + n > kWtSpan) ? -1 : s_nbnd + n;
+            if (n < kWtTPB || (round + 1) * kWtTPB >= kWtSpan + kWtTPB) break;
+        }
+    }
+    for (int i = tid; i < kWtSpan; i += kWtTPB) {
+        const int c = wide_symbol_smem(s_raw + i, prm.alphabet);
+        s_code[i] = (uint8_t)(c < 0 ? 0xFF : c);
+    }
+    __syncthreads();
+
+    // ---- B: m-mer keys, s-mer masks and k-symbol validity, rolled along kWtStrip consecutive symbols of one frame
+    {
+        const int mbits = m * b < 64 ? m * b : 64, sbits = s * b < 64 ? s * b : 64;
+        const uint64_t seedm = kSeedM & low_mask64(mbits), seeds = kSeedS & low_mask64(sbits);
+        uint32_t mmask[4], smask[4];
+        low_mask128(m * b, mmask);
+        low_mask128(s * b, smask);
+        const uint64_t kvmask = k < 64 ? ((1ull << k) - 1ull) : ~0ull;
+        const int Wd = 64 / H; // bit-slice width (A5); below 6 the salted form (A6)
+        constexpr int per_frame = (kWtSpan + NB - 1) / NB;               // symbol starts of one frame inside the span
+        constexpr int strips_per_frame = (per_frame + kWtStrip - 1) / kWtStrip;
+        auto code_at = [&](int q) -> uint32_t { return q < kWtSpan ? (uint32_t)s_code[q] : 0xFFu; };
+        for (int sidx = tid; sidx < strips_per_frame * NB; sidx += kWtTPB) {
+            const int phi = sidx % NB, j0 = (sidx / NB) * kWtStrip;
+            int q = phi + j0 * NB;
+            if (q >= kWtSpan) continue;
+            Win128 vm, vs;
+            vm.clear(); vs.clear();
+            uint64_t inv = 0; // bit i = the symbol i places before the newest of the k-symbol window is invalid
+            for (int i = 0; i < k; ++i) {
+                const uint32_t c = code_at(q + i * NB);
+                if (i < m) vm.push(c & 63u, b);
+                if (i < s) vs.push(c & 63u, b);
+                inv = (inv << 1) | (uint64_t)(c == 0xFFu);
             }
-            if (ok) {
-                const int mb = m * b < 64 ? m * b : 64, sb = s * b < 64 ? s * b : 64;
-                uint32_t minKey = 0xFFFFFFFFu;
-                for (int i = 0; i <= k - m; ++i) { // Alg. 1 l.5-9
-                    uint64_t x = wide_sub(v, k, i, m, b) ^ (kSeedM & low_mask64(mb));
-                    minKey = min(minKey, ((uint32_t)x ^ (uint32_t)(x >> 32)) * kMultG);
+            for (int j = 0; j < kWtStrip && q < kWtSpan; ++j, q += NB) {
+                const uint64_t xm = vm.fold() ^ seedm;
+                s_gk[q] = ((uint32_t)xm ^ (uint32_t)(xm >> 32)) * kMultG;
+                s_kbad[q] = (uint8_t)((inv & kvmask) != 0);
+                const uint64_t xs = vs.fold() ^ seeds;
+                uint64_t h = (xs ^ (xs >> 28)) * kMultF;
+                h ^= h >> 32;
+                uint64_t mk0 = 0, mk1 = 0, mk2 = 0, mk3 = 0;
+                if (Wd >= 6) { // A5: hash index i -> bits [i Wd, i Wd + 6) of h, word i mod 4
+                    uint64_t hh = h;
+                    for (int i = 0; i < H; i += 4) {
+                        mk0 |= 1ull << (hh & 63); hh >>= Wd;
+                        if (i + 1 < H) { mk1 |= 1ull << (hh & 63); hh >>= Wd; }
+                        if (i + 2 < H) { mk2 |= 1ull << (hh & 63); hh >>= Wd; }
+                        if (i + 3 < H) { mk3 |= 1ull << (hh & 63); hh >>= Wd; }
+                    }
+                } else {       // A6: salted upper bits
+                    for (int i = 0; i < H; ++i) {
+                        const uint64_t bit = 1ull << ((h * ((uint64_t)(2 * i + 1) * kGold64)) >> 58);
+                        if ((i & 3) == 0) mk0 |= bit; else if ((i & 3) == 1) mk1 |= bit; else if ((i & 3) == 2) mk2 |= bit; else mk3 |= bit;
+                    }
                 }
+                s_mk01[q] = make_ulonglong2(mk0, mk1);
+                s_mk23[q] = make_ulonglong2(mk2, mk3);
+                const uint32_t cm = code_at(q + m * NB), cs = code_at(q + s * NB), ck = code_at(q + k * NB);
+                vm.push(cm & 63u, b); vm.mask(mmask);
+                vs.push(cs & 63u, b); vs.mask(smask);
+                inv = (inv << 1) | (uint64_t)(ck == 0xFFu);
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- C: one k-mer per thread and byte
+    const int nbnd = s_nbnd;
+    const int nkm = k - m, nks = k - s;
+    for (int j = 0; j < kWtTile / kWtTPB; ++j) {
+        const int pr = j * kWtTPB + tid;
+        const uint64_t p = t0 + (uint64_t)pr;
+        bool present = false;
+        if (!s_kbad[pr]) { // k valid symbols from here on (bytes past the end of the buffer are invalid symbols)
+            int e_rel = 0x7FFFFFFF; // end of the record holding p, relative to t0 (no boundary inside the halo: far enough)
+            uint64_t a = 0;
+            if (prm.offsets != nullptr) {
+                if (nbnd >= 0) { // boundaries <= p among the listed ones
+                    int lo = 0, hi = nbnd;
+                    while (lo < hi) {
+                        const int mid = (lo + hi) >> 1;
+                        if ((int)s_bnd[mid] <= pr) lo = mid + 1; else hi = mid;
+                    }
+                    if (lo < nbnd) e_rel = (int)s_bnd[lo];
+                    if (NB > 1) a = lo == 0 ? s_rec0[1] : t0 + s_bnd[lo - 1];
+                } else {
+                    uint64_t lo = 0, hi = prm.n_rec;
+                    while (hi - lo > 1) {
+                        const uint64_t mid = lo + (hi - lo) / 2;
+                        if (__ldg(prm.offsets + mid) <= p) lo = mid; else hi = mid;
+                    }
+                    a = __ldg(prm.offsets + lo);
+                    const uint64_t e = __ldg(prm.offsets + lo + 1);
+                    if (e - t0 < 0x7FFFFFFFull) e_rel = (int)(e - t0);
+                }
+            }
+            bool on_grid = true; // A19: symbols sit at multiples of NB bytes from the record start
+            if (NB > 1) on_grid = (p - a + (a == 0 ? (uint64_t)prm.phase0 : 0)) % (uint64_t)NB == 0;
+            if (on_grid && pr + k * NB <= e_rel) {
+                uint32_t minKey = 0xFFFFFFFFu;
+                for (int i = 0; i <= nkm; ++i) minKey = min(minKey, s_gk[pr + i * NB]); // Alg. 1 l.5-9
                 uint64_t *sh = prm.filter + sigma_shard(minKey, prm.shard_shift) * 4;
                 uint64_t w[4] = {0, 0, 0, 0};
                 if constexpr (!INSERT) ld_shard_256(sh, w);
-                uint64_t mk[4] = {0, 0, 0, 0};
-                for (int j = 0; j <= k - s; ++j) { // Alg. 1 l.11-14 / Alg. 2 Contains
-                    uint64_t x = wide_sub(v, k, j, s, b) ^ (kSeedS & low_mask64(sb));
-                    uint64_t h = (x ^ (x >> 28)) * kMultF;
-                    h ^= h >> 32;
-                    for (int i = 0; i < H; ++i) {
-                        const uint64_t bit = 1ull << bit_pos(h, i, H);
-                        switch (i & 3) {
-                        case 0: mk[0] |= bit; break;
-                        case 1: mk[1] |= bit; break;
-                        case 2: mk[2] |= bit; break;
-                        default: mk[3] |= bit; break;
-                        }
-                    }
+                ulonglong2 m01 = make_ulonglong2(0, 0), m23 = make_ulonglong2(0, 0);
+                for (int jj = 0; jj <= nks; ++jj) { // Alg. 1 l.11-14 / Alg. 2 Contains
+                    const ulonglong2 x = s_mk01[pr + jj * NB], y = s_mk23[pr + jj * NB];
+                    m01.x |= x.x; m01.y |= x.y; m23.x |= y.x; m23.y |= y.y;
                 }
                 if constexpr (INSERT) {
-#pragma unroll
-                    for (int q = 0; q < 4; ++q)
-                        if (mk[q]) red_or_64(sh + q, mk[q]);
+                    if (m01.x) red_or_64(sh + 0, m01.x);
+                    if (m01.y) red_or_64(sh + 1, m01.y);
+                    if (m23.x) red_or_64(sh + 2, m23.x);
+                    if (m23.y) red_or_64(sh + 3, m23.y);
                 } else {
-                    present = ((mk[0] & ~w[0]) | (mk[1] & ~w[1]) | (mk[2] & ~w[2]) | (mk[3] & ~w[3])) == 0;
+                    present = ((m01.x & ~w[0]) | (m01.y & ~w[1]) | (m23.x & ~w[2]) | (m23.y & ~w[3])) == 0;
                 }
             }
         }
-    }
-    if constexpr (!INSERT) {
-        const uint32_t word = __ballot_sync(0xFFFFFFFFu, present);
-        if ((threadIdx.x & 31) == 0) {
-            const uint64_t wi = p >> 5;
-            if (wi < prm.n_bitmap_words) prm.bitmap[wi] = word;
+        if constexpr (!INSERT) {
+            const uint32_t word = __ballot_sync(0xFFFFFFFFu, present);
+            if ((tid & 31) == 0) {
+                const uint64_t wi = p >> 5;
+                if (wi < prm.n_bitmap_words) prm.bitmap[wi] = word;
+            }
         }
     }
 }

@@ -123,6 +123,28 @@ def test_unaligned_pointers_and_tiny_inputs():
     o.close()
 
 
+@pytest.mark.parametrize("alphabet,k,m,s,H", [(oracle.PROTEIN, 12, 6, 10, 4), (oracle.TRIPLET, 7, 3, 5, 4)])
+def test_more_record_boundaries_than_a_tile_lists(alphabet, k, m, s, H):
+    """wide_tile_kernel lists the record boundaries of its 1 KiB tile in shared memory; a tile crossed by thousands of
+    empty records overflows that list and must fall back to looking records up in the global offsets.  Also: records of
+    1-3 bytes (hundreds of boundaries per tile, none of them holding a k-mer) next to ordinary ones."""
+    rng = np.random.default_rng(77)
+    n = 40_000
+    text = rand_text(alphabet, 61, n)
+    text[rng.integers(0, n, 40)] = ord("#")
+    lens = []
+    left = n
+    while left > 0:
+        r = rng.random()
+        if r < 0.02:
+            lens.extend([0] * int(rng.integers(1200, 3000)))      # a burst of empty records at one position
+        l = int(min(left, rng.integers(1, 4) if r < 0.3 else rng.integers(20, 400)))
+        lens.append(l); left -= l
+    offs = np.concatenate(([0], np.cumsum(lens))).astype(np.uint64)
+    assert offs[-1] == n
+    check(alphabet, k, m, s, H, 1 << 18, text, offs, text[::-1].copy(), offs)
+
+
 @pytest.mark.parametrize("alphabet,k,m,s,H", [(oracle.TRIPLET, 10, 5, 8, 4), (oracle.DNA, 63, 31, 60, 4), (oracle.PROTEIN, 25, 7, 20, 4)])
 def test_host_facing_calls_in_several_chunks(alphabet, k, m, s, H):
     """Chunks of 1152 / 2048 bytes: k-mers straddle chunk edges (overlap k * bytes-per-symbol - 1) and, for triplets,
