@@ -1174,7 +1174,7 @@ __device__ __forceinline__ int dna_code(uint32_t c)
 //   C  one k-mer per thread and byte: validity from the record boundaries, the symbol grid and the rolled invalid
 //      flag, minimum of k-m+1 keys, OR of k-s+1 mask quadruples — then the shard update / test of Alg. 1 / Alg. 2.
 //      A warp covers 32 consecutive bytes: the query result word is one ballot.
-// 2.2-4.9 x the one-k-mer-per-thread form (protein k=12: 51, k=25: 43, triplets k=10: 14, DNA k=63 without a
+// 2.2-4.9 x the one-k-mer-per-thread form (protein k=12: 51, k=25: 43, triplets k=10: 16, DNA k=63 without a
 // specialised instance: 31 G k-mers/s on 60 MB).  A tile with more record boundaries than it has room for (thousands
 // of empty records in 1 KiB) looks its records up in global memory instead.
 // ---------------------------------------------------------------------------------------------
@@ -1229,6 +1229,7 @@ __global__ void __launch_bounds__(kWtTPB) wide_tile_kernel(const WideParams prm)
     __shared__ uint8_t s_kbad[kWtSpan];                   // the k symbols starting at each byte hold an invalid one
     __shared__ uint64_t s_rec0[2];                        // index and start of the record holding byte t0
     __shared__ int s_nbnd;                                // boundaries listed; -1: too many, look records up globally
+    __shared__ unsigned s_frames;                         // NB > 1: bit f = some record of the tile has its symbol grid on frame f
 
     const int k = prm.k, m = prm.m, s = prm.s, H = prm.H, b = prm.sym_bits;
     const int tid = threadIdx.x;
@@ -1257,6 +1258,7 @@ __global__ void __launch_bounds__(kWtTPB) wide_tile_kernel(const WideParams prm)
             s_rec0[0] = lo;
             s_rec0[1] = prm.offsets != nullptr ? __ldg(prm.offsets + lo) : 0;
             s_nbnd = 0;
+            s_frames = 0;
         }
     }
     __syncthreads();
@@ -1278,6 +1280,18 @@ __global__ void __launch_bounds__(kWtTPB) wide_tile_kernel(const WideParams prm)
         const int c = wide_symbol_smem(s_raw + i, prm.alphabet);
         s_code[i] = (uint8_t)(c < 0 ? 0xFF : c);
     }
+    if (NB > 1) { // which of the NB frames (byte position mod NB inside the tile) carry some record's symbol grid (A19)
+        const int nb_listed = s_nbnd;
+        if (nb_listed < 0) {
+            if (tid == 0) s_frames = (1u << NB) - 1u;
+        } else {
+            for (int i = tid; i <= nb_listed; i += kWtTPB) { // record 0 of the tile, then the records starting at the boundaries
+                const uint64_t a = i == 0 ? s_rec0[1] : t0 + s_bnd[i - 1];
+                const unsigned ph = a == 0 ? (unsigned)prm.phase0 % NB : 0u;
+                atomicOr(&s_frames, 1u << (((unsigned)(a % NB) + 2u * NB - ph - (unsigned)(t0 % NB)) % NB));
+            }
+        }
+    }
     __syncthreads();
 
     // ---- B: m-mer keys, s-mer masks and k-symbol validity, rolled along kWtStrip consecutive symbols of one frame
@@ -1293,9 +1307,10 @@ __global__ void __launch_bounds__(kWtTPB) wide_tile_kernel(const WideParams prm)
         constexpr int strips_per_frame = (per_frame + kWtStrip - 1) / kWtStrip;
         auto code_at = [&](int q) -> uint32_t { return q < kWtSpan ? (uint32_t)s_code[q] : 0xFFu; };
         for (int sidx = tid; sidx < strips_per_frame * NB; sidx += kWtTPB) {
-            const int phi = sidx % NB, j0 = (sidx / NB) * kWtStrip;
+            const int phi = sidx / strips_per_frame, j0 = (sidx % strips_per_frame) * kWtStrip; // frame-major: whole warps skip a dead frame
             int q = phi + j0 * NB;
             if (q >= kWtSpan) continue;
+            if (NB > 1 && !((s_frames >> phi) & 1u)) continue; // no record of this tile has a k-mer on this frame
             Win128 vm, vs;
             vm.clear(); vs.clear();
             uint64_t inv = 0; // bit i = the symbol i places before the newest of the k-symbol window is invalid
