@@ -9,8 +9,12 @@
 //                          next k, or fewer than k symbols left)
 //   mark_ends_kernel   a1  chunk mode over records: ORs into V the k-1 start positions before every record
 //                          end (a k-mer never spans two records)
-//   stream_kernel      a2-a6  the fused, thread-serial streaming insert / query kernel
+//   stream_kernel      a2-a6  the fused, thread-serial streaming insert / query kernel (chunk mode)
+//   stream_rec_kernel  a2-a6  the same query pipeline, one thread per short record (record mode)
+//                          query test: SlidingGather (byte-gather form, H <= 4) or SlidingOr (256-bit masks)
 //   naive_kernel       a2-a6  runtime-parameter one-k-mer-per-thread form of Alg. 1/2 (any legal k,m,s,H)
+//   wide_tile_kernel   a1-a6  the other alphabets and DNA k > 32 without an instance, from the ASCII bytes,
+//                          runtime parameters, a tile of 1024 byte positions per CTA through shared memory
 //   count kernels      a6  per-record / total popcount of the result bitmap
 #pragma once
 
