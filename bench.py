@@ -626,7 +626,7 @@ def measure_ceilings(sbf, filter_bytes, gpu_index, sm_max_mhz):
         clocks[name] = mhz
         per_clk[name] = g_per_s * 1e3 / (mhz if mhz else sm_max_mhz)
     names = ["red_or_b64_x4", "red_or_b64_x1", "ld_nc_256", "cp_async_2x16", "tma_reduce_or_32B", "ld_nc_256_L2_64B",
-             "cp_async_2x16_L2_64B"]
+             "cp_async_2x16_L2_64B", "st_256"]
     rnd = {}
     for mode, nm in enumerate(names):
         try:

@@ -236,7 +236,8 @@ int sbf_get_timing(sbf_t *f, float *ms3);
  *   array_bytes (rounded down to a power of two), allocated and freed inside the call.  mode 0: 4 x red.or.b64 per
  *   sector (the insert kernel's flush), 1: 1 x red.or.b64, 2: one 256-bit ld.global.nc, 3: 2 x 16-byte cp.async into
  *   shared memory, 4: one 32-byte cp.reduce.async.bulk .or.b64 (TMA reduction), 5: mode 2 with the .L2::64B
- *   prefetch-size hint, 6: mode 3 with the .L2::64B hint (the query kernels' staging, exactly).
+ *   prefetch-size hint, 6: mode 3 with the .L2::64B hint (the query kernels' staging, exactly), 7: one plain 256-bit
+ *   st.global of the whole sector (no fetch needed).
  * Both synchronise the device.
  */
 int sbf_ceiling_pipe_modes(void);

@@ -26,7 +26,7 @@ def main():
         for mode in range(sbf.sbf_ceiling_pipe_modes()):
             out["pipe_g_warp_inst_per_s_per_smsp"][sbf.sbf_ceiling_pipe_mode_name(mode)] = sbf.sbf_ceiling_pipe_rate(mode, args.iters)[0]
     for mode, name in enumerate(["red_or_b64_x4", "red_or_b64_x1", "ld_nc_256", "cp_async_2x16", "tma_reduce_or_32B",
-                                 "ld_nc_256_L2_64B", "cp_async_2x16_L2_64B"]):
+                                 "ld_nc_256_L2_64B", "cp_async_2x16_L2_64B", "st_256"]):
         out["random_sector_g_per_s"][name] = sbf.sbf_ceiling_random_sector(mode, args.bytes)
     print(json.dumps(out))
     return 0

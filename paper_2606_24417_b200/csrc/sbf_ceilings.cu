@@ -94,6 +94,7 @@ __device__ __forceinline__ uint64_t mix64(uint64_t x)
 //      4: one 32-byte cp.reduce.async.bulk .or.b64 from shared memory (TMA reduction) per random sector
 //      5: mode 2 with the .L2::64B prefetch-size hint (a miss pulls 64 B from DRAM instead of 128 B)
 //      6: mode 3 with the .L2::64B hint (exactly what the query kernels issue per run)
+//      7: one plain 256-bit st.global of a whole random sector (a write needs no fetch: one DRAM transaction)
 constexpr int kRandTPB = 128;
 template <int MODE>
 __global__ void __launch_bounds__(kRandTPB) random_sector_kernel(uint64_t *arr, uint64_t sector_mask, uint32_t per_thread, uint64_t *sink)
@@ -115,6 +116,8 @@ __global__ void __launch_bounds__(kRandTPB) random_sector_kernel(uint64_t *arr, 
             uint64_t w0, w1, w2, w3;
             asm volatile("ld.global.nc.v4.u64 {%0,%1,%2,%3}, [%4];" : "=l"(w0), "=l"(w1), "=l"(w2), "=l"(w3) : "l"(p));
             acc += w0 ^ w1 ^ w2 ^ w3;
+        } else if (MODE == 7) {
+            asm volatile("st.global.v4.u64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(v), "l"(v << 1), "l"(v >> 1), "l"(v | 1) : "memory");
         } else if (MODE == 5) {
             uint64_t w0, w1, w2, w3;
             asm volatile("ld.global.nc.L2::64B.v4.u64 {%0,%1,%2,%3}, [%4];" : "=l"(w0), "=l"(w1), "=l"(w2), "=l"(w3) : "l"(p));
@@ -227,7 +230,7 @@ int sbf_ceiling_pipe_rate(int mode, int iters, double *g_warp_inst_per_s_per_sms
 
 int sbf_ceiling_random_sector(int mode, uint64_t array_bytes, double *g_accesses_per_s)
 {
-    if (mode < 0 || mode > 6 || !g_accesses_per_s || array_bytes < 4096) return SBF_ERR_INVALID_ARG;
+    if (mode < 0 || mode > 7 || !g_accesses_per_s || array_bytes < 4096) return SBF_ERR_INVALID_ARG;
     uint64_t sectors = 1;
     while (sectors * 2 * 32 <= array_bytes) sectors *= 2; // power of two
     int dev = 0, sms = 0;
@@ -255,7 +258,8 @@ int sbf_ceiling_random_sector(int mode, uint64_t array_bytes, double *g_accesses
         case 3: err = launch_rand<3>(arr, sectors - 1, per_thread, sink, blocks); break;
         case 4: err = launch_rand<4>(arr, sectors - 1, per_thread, sink, blocks); break;
         case 5: err = launch_rand<5>(arr, sectors - 1, per_thread, sink, blocks); break;
-        default: err = launch_rand<6>(arr, sectors - 1, per_thread, sink, blocks); break;
+        case 6: err = launch_rand<6>(arr, sectors - 1, per_thread, sink, blocks); break;
+        default: err = launch_rand<7>(arr, sectors - 1, per_thread, sink, blocks); break;
         }
         cudaEventRecord(e1);
         if (err == cudaSuccess) err = cudaEventSynchronize(e1);

@@ -65,7 +65,7 @@ def test_pipe_rate_loop_bodies_are_counted_in_sass():
 
 def test_random_sector_kernels_issue_the_named_access():
     hist = _histograms()
-    want = {0: "REDG", 1: "REDG", 2: "LDG", 3: "LDGSTS", 4: "UBLKRED", 5: "LDG", 6: "LDGSTS"}
+    want = {0: "REDG", 1: "REDG", 2: "LDG", 3: "LDGSTS", 4: "UBLKRED", 5: "LDG", 6: "LDGSTS", 7: "STG"}
     for fn, h in hist.items():
         m = re.search(r"random_sector_kernelILi(\d+)E", fn)
         if m:
