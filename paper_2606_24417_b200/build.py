@@ -45,8 +45,13 @@ def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str =
     srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
     if not srcs:
         raise RuntimeError("no CUDA sources under %s" % CSRC)
-    os.makedirs(objdir, exist_ok=True)
     hdr_time = max(os.path.getmtime(h) for h in _headers())
+    # a library newer than every source and header is current even when the objects are gone (they do not travel to the
+    # GPU box: .gpurunignore): nothing to do
+    if not force and os.path.exists(lib) and os.path.getmtime(lib) >= max([hdr_time] + [os.path.getmtime(x) for x in srcs]) \
+            and os.path.getmtime(lib) >= os.path.getmtime(os.path.abspath(__file__)):
+        return lib
+    os.makedirs(objdir, exist_ok=True)
     nvcc = _nvcc()
     jobs = []
     objs = []
