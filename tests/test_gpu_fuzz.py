@@ -22,7 +22,7 @@ def _random_sequence(rng, n):
     lower = rng.random(n) < 0.2
     seq[lower] |= 0x20
     if rng.random() < 0.5:                                          # a low-complexity stretch
-        a = int(rng.integers(0, max(1, n - 3000))); seq[a:a + 3000] = np.frombuffer(b"ACAC" * 750, dtype=np.uint8)
+        a = int(rng.integers(0, max(1, n - 3000))); seq[a:a + 3000] = np.frombuffer(b"ACAC" * 750, dtype=np.uint8)[:seq[a:a + 3000].size]
     return seq
 
 
