@@ -1017,16 +1017,17 @@ __global__ void __launch_bounds__(kRecTPB, SBF_MINB_R) stream_rec_kernel(const S
     // result bits leave through a 64-bit buffer aligned to the bitmap's words
     uint64_t rb = 0;
     uint32_t fill = (uint32_t)(a & 31), cnt = 0;
-    uint64_t wi = a >> 5;
-    bool first = true;
+    uint32_t *bw = prm.bitmap + (a >> 5);                      // the bitmap word being filled
+    const uint32_t w_shared = (uint32_t)((e >> 5) - (a >> 5)); // words from this index on reach past the record's end
+    uint32_t wrel = 0;
     auto emit = [&](uint32_t word) {
-        if (first || (wi + 1) * 32 > e) {
-            if (word) atomicOr(prm.bitmap + wi, word);
+        if (wrel == 0 || wrel >= w_shared) { // shared with a neighbouring record (or the first word: a is rarely 32-aligned)
+            if (word) atomicOr(bw, word);
         } else {
-            prm.bitmap[wi] = word;
+            *bw = word;
         }
-        first = false;
-        ++wi;
+        ++bw;
+        ++wrel;
     };
 
     const uint32_t nblk = (nk + 15) >> 4;
