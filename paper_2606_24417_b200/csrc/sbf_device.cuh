@@ -78,7 +78,10 @@ constexpr uint64_t kMultF = 0xD6E8FEB86659FD93ull;
 
 // ---- launch geometry ---------------------------------------------------------------------
 constexpr int kChunk = 128;     // most k-mer start positions walked by one thread of stream_kernel (StreamParams::chunk_blocks * 16)
-constexpr int kStreamTPB = 128; // threads per CTA of stream_kernel
+#ifndef SBF_STREAM_TPB
+#define SBF_STREAM_TPB 128
+#endif
+constexpr int kStreamTPB = SBF_STREAM_TPB; // threads per CTA of stream_kernel
 #ifndef SBF_REC_TPB
 #define SBF_REC_TPB 128
 #endif
@@ -355,7 +358,7 @@ __global__ void __launch_bounds__(256) mark_ends_kernel(const uint64_t *__restri
 // 64 bits as A21 prescribes (its last 32 symbols XOR the rotated golden-ratio multiple of the symbols before them).
 // All shifts are immediates.  NWIN = 4 up to k = 42, 5 up to k = 58, 6 up to k = 64 (kWinOf).
 // =============================================================================================
-__host__ __device__ constexpr int kWinOf(int K) { return (K + 22 + 15) / 16 < 4 ? 4 : (K + 22 + 15) / 16; } // 15 + look-ahead 7 + k symbols
+__host__ __device__ constexpr int kWinOf(int K) { return (K + 15 + SBF_Q_LA + 15) / 16 < 4 ? 4 : (K + 15 + SBF_Q_LA + 15) / 16; } // 15 + look-ahead + k symbols
 
 template <int Q, int NB, int NWIN>
 __device__ __forceinline__ uint32_t field_win(const uint32_t (&W)[NWIN])
