@@ -64,7 +64,7 @@
 #define SBF_MINB_I 5 // insert: CTAs per SM the register budget is cut for (5 x 128 threads -> 96 registers)
 #endif
 #ifndef SBF_MINB_Q
-#define SBF_MINB_Q 4 // chunk-mode query: 4 x 128 threads -> 128 registers (5 -> 96 registers spills: 0.333 vs 0.328 ms per 100 Mbp)
+#define SBF_MINB_Q 5 // chunk-mode query: 5 x 128 threads -> 96 registers (with the byte-gather state: 0.632 vs 0.640 ms per 240 Mbp at 4 CTAs; the mask form spilled at 96)
 #endif
 
 namespace sbfk {
