@@ -64,7 +64,7 @@
 #define SBF_MINB_I 5 // insert: CTAs per SM the register budget is cut for (5 x 128 threads -> 96 registers)
 #endif
 #ifndef SBF_MINB_Q
-#define SBF_MINB_Q 5 // chunk-mode query, byte-gather form: 5 x 128 threads -> 96 registers (0.632 vs 0.640 ms per 240 Mbp at 4 CTAs); the mask form spills at 96 and stays at 4 x 128 threads -> 128 registers
+#define SBF_MINB_Q 5 // chunk-mode query, byte-gather form: 5 x 128 threads -> 96 registers (0.632 vs 0.640 ms per 240 Mbp at 4 CTAs); the mask form and the wider windows of k > 32 spill at 96 and stay at 4 x 128 threads -> 128 registers
 #endif
 
 namespace sbfk {
@@ -829,7 +829,7 @@ struct QueryLane {
 // read-modify-write serves; slower while the filter is L2-resident, where the TMA unit's ~24 G operations/s cap binds).
 constexpr int kModeQuery = 0, kModeInsert = 1, kModeInsertTma = 2;
 template <int K, int M, int S, int H, int MODE>
-__global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : (gather_form<K - S + 1, H>() ? SBF_MINB_Q : 4))
+__global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : (gather_form<K - S + 1, H>() && K <= 32 ? SBF_MINB_Q : 4))
     stream_kernel(const StreamParams prm)
 {
     constexpr bool INSERT = MODE != kModeQuery;
