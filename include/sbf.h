@@ -207,6 +207,54 @@ int sbf_ipc_export_filter(const sbf_t *f, void *handle64);
 int sbf_ipc_open_filter(const void *handle64, uint64_t **d_ptr);
 int sbf_ipc_close_filter(uint64_t *d_ptr);
 
+/*
+ * sbf_query_seq_static — sbf_query_seq (Alg. 2) for callers that must not allocate device memory.
+ *
+ * Who this is for.  A query needs working memory besides its input and output: the 2-bit packed copy of the sequence
+ * and its validity mask (0.375 bytes per symbol), which the handle-based calls cudaMalloc and grow on demand.  Some
+ * programs cannot let a library do that: a service whose device memory was handed out in full to its own arena or to a
+ * framework's caching allocator at start-up (a cudaMalloc from a library then fails, or steals from that pool); a
+ * latency-bound loop that cannot take the device-wide synchronisation a cudaMalloc / cudaFree implies; a plug-in that
+ * runs under a fixed per-process memory budget (MPS / MIG partitions) and may only use what its host hands it.  Such a
+ * caller keeps the filter in memory of its own and calls this one function: no handle, no cudaMalloc, cudaFree,
+ * cudaMallocAsync or any other allocating routine, on any call.
+ *
+ * Working memory.  The packed copy and the mask live in ONE array of device memory compiled into the library
+ * (6 MiB + 512 bytes, file scope in sbf_api.cu).  Every GPU whose context loads libsbf_b200.so holds that array from module
+ * load until the process exits, whether or not this function is ever called.  Its size fixes the limit:
+ *   len <= SBF_STATIC_MAX_SYMBOLS (2^24 = 16 Mi symbols per call); a longer sequence is rejected with
+ *   SBF_ERR_INVALID_ARG and a message that names the limit — split it into pieces that overlap by k-1 symbols.
+ *
+ * Arguments (all device pointers are the caller's, on the CURRENT device):
+ *   k, m, s, H      as sbf_create; DNA alphabet only.  k <= 32, or 33 <= k <= 64 where a streaming instance is compiled;
+ *                   anything else is SBF_ERR_UNSUPPORTED (the other alphabets' kernel needs no working memory at all,
+ *                   so sbf_query_seq on a handle already allocates nothing for them).
+ *   d_filter        the filter in layout A12: num_shards x 32 bytes, 32-byte aligned, read only.  num_shards is a power
+ *                   of two, at most 2^32, and must be the shard count the bits were inserted with.  Either memory the
+ *                   caller filled itself (e.g. from sbf_export_bits of another process) or sbf_filter_device_ptr() /
+ *                   sbf_num_shards() of a handle created while allocating was still allowed.
+ *   d_seq, len      the ASCII symbols, as sbf_query_seq.  len may be 0 (nothing is enqueued).
+ *   d_bitmap        ceil(len/32) uint32 words, all written; bit p as in sbf_query_seq.
+ *   stream          the work is enqueued on it and the call returns without synchronising.
+ *
+ * Set-up.  The FIRST call on each device looks up the device address of the array (once per device, with that device
+ * current; the result is cached) before it enqueues anything.  Make that first call outside any stream capture, e.g.
+ * with len = 0 at start-up; later calls on the same device only launch kernels.
+ *
+ * Sharing.  All calls in the process — every thread, every stream, every filter — use the same array, and it keeps
+ * whatever the previous call left in it.  That is harmless in sequence: the packing step rewrites every word the query
+ * step reads before it reads it, so nothing has to start at zero and nothing is cleared.  It is NOT harmless in
+ * parallel: two calls whose kernels may overlap on one GPU (different streams, or different host threads) race on the
+ * array and both results are undefined.  Order such calls on one stream or with events.  Calls on different GPUs do not
+ * interact (each GPU has its own copy).  The handle-based calls never touch this array.
+ *
+ * Result: bit-identical to sbf_query_seq on a handle with the same (k,m,s,H) and filter contents.  The L2 persistence
+ * window of a7 is not applied (stream attributes are left alone).
+ */
+#define SBF_STATIC_MAX_SYMBOLS (1ull << 24)
+int sbf_query_seq_static(int k, int m, int s, int H, const uint64_t *d_filter, uint64_t num_shards, const char *d_seq,
+                         uint64_t len, uint32_t *d_bitmap, void *stream);
+
 /* Message for the last error on the calling thread ("" if none). */
 const char *sbf_last_error(void);
 

@@ -41,6 +41,7 @@ ABI = {
     "sbf_insert_records": (_i32, [_p, _p, _p, _u64, _u64, _p]),
     "sbf_query_seq": (_i32, [_p, _p, _u64, _p, _p, _p]),
     "sbf_query_records": (_i32, [_p, _p, _p, _u64, _u64, _p, _p, _p]),
+    "sbf_query_seq_static": (_i32, [_i32, _i32, _i32, _i32, _p, _u64, _p, _u64, _p, _p]),
     "sbf_insert_seq_host": (_i32, [_p, _p, _u64]),
     "sbf_insert_records_host": (_i32, [_p, _p, _p, _u64]),
     "sbf_query_seq_host": (_i32, [_p, _p, _u64, _p, _p]),
@@ -190,6 +191,19 @@ def sbf_query_seq(h, d_seq, length: int, d_bitmap, d_hits=None, stream=None):
 def sbf_query_records(h, d_bases, d_offsets, n_rec: int, total_bases: int, d_bitmap, d_hit_counts=None, stream=None):
     _check(load_library().sbf_query_records(h, _dptr(d_bases), _dptr(d_offsets), n_rec, total_bases, _dptr(d_bitmap),
                                             _dptr(d_hit_counts), _stream(stream)))
+
+
+STATIC_MAX_SYMBOLS = 1 << 24  # SBF_STATIC_MAX_SYMBOLS of include/sbf.h
+
+
+def sbf_query_seq_static(k: int, m: int, s: int, H: int, d_filter, num_shards: int, d_seq, length: int, d_bitmap, stream=None):
+    """sbf_query_seq without a handle and without any device allocation, for callers that may not allocate (a process
+    whose device memory belongs to its own pool, a loop that cannot take cudaMalloc's synchronisation): the working
+    memory is one fixed array inside the library, shared by every call, so at most STATIC_MAX_SYMBOLS symbols per call
+    and never two calls in flight at once on one GPU.  d_filter: the caller's filter (layout A12, num_shards x 32 bytes).
+    See include/sbf.h."""
+    _check(load_library().sbf_query_seq_static(k, m, s, H, _dptr(d_filter), num_shards, _dptr(d_seq), length,
+                                               _dptr(d_bitmap), _stream(stream)))
 
 
 def sbf_insert_seq_host(h, h_seq, length: int):

@@ -8,6 +8,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1106,6 +1107,126 @@ int sbf_query_fastx_host(sbf_t *f, const char *h_text, uint64_t n_bytes, int for
 {
     if (!f || (!h_text && n_bytes)) return fail(SBF_ERR_INVALID_ARG, "sbf_query_fastx_host: NULL argument");
     return run_fastx(f, false, h_text, n_bytes, format, h_hit_counts, h_hit_counts ? max_records : 0, n_records, n_bases);
+}
+
+} // extern "C"
+
+// =============================================================================================
+// sbf_query_seq_static (include/sbf.h): the sequence query for callers that may not allocate device memory.
+// Same two launches as sbf_query_seq on a handle — pack_kernel, then the chunk-mode query kernel — but the packed
+// words and the validity mask go to an array that is part of the library image instead of cudaMalloc'ed scratch.
+// =============================================================================================
+namespace {
+constexpr uint64_t kStaticMaxSymbols = SBF_STATIC_MAX_SYMBOLS;
+constexpr uint64_t kStaticWords = (kStaticMaxSymbols + 15) / 16 + kPadWords;             // what pack_kernel writes at the limit
+constexpr uint64_t kStaticPackedBytes = (kStaticWords * sizeof(uint32_t) + 255) / 256 * 256;
+constexpr uint64_t kStaticMaskBytes = (kStaticWords * sizeof(uint16_t) + 8 + 255) / 256 * 256; // + 8 as ensure_scratch: the last mask store is 4 bytes wide
+constexpr uint64_t kStaticBytes = kStaticPackedBytes + kStaticMaskBytes;                   // 6 MiB + 512 B
+} // namespace
+
+// The working memory itself: [0, kStaticPackedBytes) packed words, then the mask.  Every device that loads this
+// module holds one copy until the process exits.  In host code this name is only a handle for the runtime's symbol
+// table — never a device address, so it is never passed to a kernel; static_scratch() below asks the runtime
+// where the current device keeps its copy.
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticBytes];
+
+namespace {
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+unsigned char *g_static_ptr[kStaticMaxDevices]; // device address of g_static_scratch on device i, once looked up
+
+// Device address of the array on the CURRENT device.  First call per device: one cudaGetSymbolAddress (it allocates
+// nothing — the array came with the module — but it may make the runtime finish loading the module, which is why the
+// header asks for the first call outside stream capture).  Later calls: a table read.
+int static_scratch(unsigned char **out)
+{
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices)
+        return fail(SBF_ERR_UNSUPPORTED, "sbf_query_seq_static: device ordinal above 63");
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (g_static_ptr[dev] == nullptr) {
+        void *p = nullptr;
+        CK(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (p == nullptr) return fail(SBF_ERR_CUDA, "sbf_query_seq_static: the runtime returned no address for the static scratch array");
+        g_static_ptr[dev] = static_cast<unsigned char *>(p);
+    }
+    *out = g_static_ptr[dev];
+    return SBF_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int sbf_query_seq_static(int k, int m, int s, int H, const uint64_t *d_filter, uint64_t num_shards, const char *d_seq,
+                         uint64_t len, uint32_t *d_bitmap, void *stream)
+{
+    if (k < 1 || k > 64 || m < 1 || m > k || s < 1 || s > k || H < 1 || H > 32)
+        return fail(SBF_ERR_INVALID_ARG, "sbf_query_seq_static: need 1<=k<=64, 1<=m<=k, 1<=s<=k, 1<=H<=32");
+    if (num_shards == 0 || (num_shards & (num_shards - 1)) != 0 || num_shards > (1ull << 32))
+        return fail(SBF_ERR_INVALID_ARG, "sbf_query_seq_static: num_shards must be a power of two, at most 2^32");
+    if (!d_filter || (reinterpret_cast<uintptr_t>(d_filter) & 31) != 0)
+        return fail(SBF_ERR_INVALID_ARG, "sbf_query_seq_static: d_filter is NULL or not 32-byte aligned");
+    if ((!d_seq && len) || (!d_bitmap && len)) return fail(SBF_ERR_INVALID_ARG, "sbf_query_seq_static: NULL argument");
+    if (len > kStaticMaxSymbols) {
+        char msg[224];
+        snprintf(msg, sizeof(msg),
+                 "sbf_query_seq_static: len = %llu symbols is above the static scratch limit SBF_STATIC_MAX_SYMBOLS = %llu; "
+                 "split the sequence into pieces that overlap by k-1 symbols",
+                 (unsigned long long)len, (unsigned long long)kStaticMaxSymbols);
+        return fail(SBF_ERR_INVALID_ARG, msg);
+    }
+    int P = 0;
+    while ((1ull << P) < num_shards) ++P;
+    // same routing as sbf_create: a compiled instance where there is one (they take sigma's shift as a multiply by
+    // 2^P, hence P < 32), else the runtime-parameter kernel, which packs a k-mer into one 64-bit word
+    const KernelEntry *entry = P < 32 ? find_entry(k, m, s, H) : nullptr;
+    if (entry == nullptr && k > 32)
+        return fail(SBF_ERR_UNSUPPORTED, "sbf_query_seq_static: no streaming instance for this k > 32 (or 2^32 shards); use a handle");
+
+    // set-up comes before the len == 0 exit so that an empty call at start-up does it
+    unsigned char *scratch = nullptr;
+    int rc = static_scratch(&scratch);
+    if (rc) return rc;
+    if (len == 0) return SBF_OK;
+
+    cudaStream_t st = (cudaStream_t)stream;
+    uint32_t *packed = reinterpret_cast<uint32_t *>(scratch);
+    uint16_t *vmask = reinterpret_cast<uint16_t *>(scratch + kStaticPackedBytes);
+    // a1: every word the query kernel will read (the pad words included) is rewritten here, so what the previous call
+    // left in the array never reaches a result
+    const uint64_t nw = (len + 15) / 16 + kPadWords;
+    const unsigned pack_blocks = (unsigned)(((nw + 1) / 2 + 255) / 256);
+    const int aligned = ((reinterpret_cast<uintptr_t>(d_seq) & 15) == 0) ? 1 : 0;
+    pack_kernel<<<pack_blocks, 256, 0, st>>>(reinterpret_cast<const uint8_t *>(d_seq), len, packed, vmask, nw, k, aligned, nullptr,
+                                             (len + 31) / 32, nullptr);
+    CK(cudaGetLastError());
+    g_launches++;
+
+    // a2-a6: chunk-mode query, parameters as make_params() sets them for a handle
+    StreamParams p;
+    p.packed = packed;
+    p.vmask = vmask;
+    p.n_pos = len;
+    p.filter = const_cast<uint64_t *>(d_filter); // the query kernels only load from it
+    p.shard_shift = 32 - P;
+    p.bitmap = d_bitmap;
+    p.n_bitmap_words = (len + 31) / 32;
+    p.chunk_blocks = len >= (64ull << 20) ? 8 : len >= (16ull << 20) ? 4 : 2;
+    p.offsets = nullptr; p.n_rec = 0; p.counts = nullptr; p.fallback = nullptr; p.rec_limit = 0;
+    if (entry) {
+        CK(entry->query(p, st));
+    } else {
+        NaiveParams np;
+        np.sp = p; np.k = k; np.m = m; np.s = s; np.H = H;
+        const uint64_t n32 = (len + 31) / 32 * 32;
+        naive_kernel<false><<<(unsigned)((n32 + 255) / 256), 256, 0, st>>>(np);
+        CK(cudaGetLastError());
+    }
+    g_launches++;
+    return SBF_OK;
 }
 
 } // extern "C"
