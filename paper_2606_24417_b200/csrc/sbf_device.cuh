@@ -1290,6 +1290,7 @@ __global__ void __launch_bounds__(kWtTPB) wide_tile_kernel(const WideParams prm)
         s_code[i] = (uint8_t)(c < 0 ? 0xFF : c);
     }
     if (NB > 1) { // which of the NB frames (byte position mod NB inside the tile) carry some record's symbol grid (A19)
+        __syncthreads(); // thread 0 wrote s_nbnd after the boundary loop's last barrier: order that write before the reads below
         const int nb_listed = s_nbnd;
         if (nb_listed < 0) {
             if (tid == 0) s_frames = (1u << NB) - 1u;
