@@ -157,7 +157,8 @@ int sbf_query_records_host(sbf_t *f, const char *h_bases, const uint64_t *h_offs
  *   Text rules: lines end at '\n'; '\r' is dropped; FASTA: a line starting with '>' is a header and starts a
  *   record, every other line is sequence of the current record (text before the first header is inserted by the
  *   insert call and ignored by the query call); FASTQ: four lines per record (header, sequence, '+', quality;
- *   multi-line FASTQ is not supported).  Sequence bytes are taken verbatim: validity is the alphabet's (A9 / A19).
+ *   multi-line FASTQ is not supported); a record starts at a line of index 0 mod 4 whose first byte is neither '\n'
+ *   nor '\r' — a blank line, e.g. the last one of a text ending in "\n\n", counts as a line but opens no record.  Sequence bytes are taken verbatim: validity is the alphabet's (A9 / A19).
  * The raw text is copied to the device in chunks of sbf_set_host_chunk() bytes on one stream while the previous
  * chunk is normalised ON THE DEVICE (headers, quality and line ends dropped, records compacted into a dense batch +
  * offsets) and inserted / queried on another; records and k-mers may straddle chunk edges.  Synchronises.

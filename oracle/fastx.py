@@ -6,7 +6,8 @@ stated in include/sbf.h): lines end at '\\n'; '\\r' is dropped; every other byte
   FASTA  a line whose first byte is '>' is a header and starts a record; every other line belongs to the current
          record; text before the first header is the `pre` segment (inserted by the insert call, ignored by queries).
   FASTQ  four lines per record: header, sequence, '+', quality (line index mod 4); a record starts at a line with
-         index 0 mod 4 that holds at least one byte.
+         index 0 mod 4 whose first byte is neither '\\n' nor '\\r' (A23: a blank line, e.g. the one a
+         text ending in two newlines has, still counts as a line but opens no record).
 Shares nothing with the CUDA path and never imports it.
 """
 from __future__ import annotations
@@ -38,7 +39,7 @@ def parse(text: bytes, fmt: int = 0):
     else:
         for idx, raw in enumerate(lines):
             if idx % 4 == 0:
-                if len(raw) > 0:
+                if raw[:1] not in (b"", b"\r"):
                     records.append(bytearray())
             elif idx % 4 == 1:
                 if records:

@@ -10,7 +10,8 @@
 //   FASTA  a line whose first byte is '>' is a header and starts a record; all other lines are sequence lines of the
 //          current record (bytes before the first header belong to "record 0" of the chunk, see below)
 //   FASTQ  four lines per record: header, sequence, '+', quality (line index mod 4; multi-line FASTQ is not supported);
-//          a record starts at the first byte of a line with index = 0 mod 4
+//          a record starts at the first byte of a line with index = 0 mod 4, unless that byte is '\n' or '\r' (a blank
+//          line, e.g. the second '\n' of a text ending in "\n\n", still counts as a line but opens no record)
 // One chunk of text yields: dense bytes [carry | sequence bytes of the chunk], offsets[0] = 0, one offset per record
 // start, offsets[n_rec] = n_bases, with n_rec = 1 + record starts: local record 0 is whatever precedes the first
 // record start of the chunk — the continuation of the previous chunk's last record, led by its last k-1 bytes (the
@@ -47,8 +48,8 @@ struct FastxState {          // device-resident, carried from one chunk to the n
 //   FASTA: has_ls/last_hdr = the stretch contains a line start / its last line start is a header; pre = non-EOL bytes
 //          before the first line start (sequence iff the stretch is entered outside a header); post = sequence bytes
 //          after it (decided locally); starts = header line starts.
-//   FASTQ: nl = newlines; seq[r] = non-EOL bytes on lines whose local index is r mod 4; ls[r] = line starts with local
-//          index r mod 4 (local index = newlines before the byte).
+//   FASTQ: nl = newlines; seq[r] = non-EOL bytes on lines whose local index is r mod 4; ls[r] = starts of non-blank lines with
+//          local index r mod 4 (local index = newlines before the byte).
 struct Seg {
     uint32_t has_ls, last_hdr, pre, post, starts; // FASTA
     uint32_t nl, seq[4], ls[4];                   // FASTQ
@@ -132,7 +133,7 @@ __device__ __forceinline__ Seg seg_of(const uint8_t *__restrict__ text, uint64_t
                 else if (!hdr_line) ++s.post;
             }
         } else {
-            if (ls) ++s.ls[s.nl & 3];
+            if (ls && !fx_is_eol(c)) ++s.ls[s.nl & 3]; // a blank line opens no record
             if (!fx_is_eol(c)) ++s.seq[s.nl & 3];
             if (c == '\n') ++s.nl;
         }
@@ -251,7 +252,7 @@ __global__ void __launch_bounds__(kFxThreads) fastx_emit_kernel(const uint8_t *_
             }
             is_seq = !in_hdr && !fx_is_eol(c);
         } else {
-            if (ls && line == 0) offsets[1 + rec++] = pos;
+            if (ls && line == 0 && !fx_is_eol(c)) offsets[1 + rec++] = pos;
             is_seq = line == 1 && !fx_is_eol(c);
             if (c == '\n') line = (line + 1) & 3;
         }

@@ -110,6 +110,35 @@ def test_fasta_other_alphabets_and_wide_kmers(alphabet, params):
         o.close()
 
 
+@pytest.mark.parametrize("chunk", [1152, 0])
+@pytest.mark.parametrize("tail", [b"\n\n", b"\n\n\n\n", b"\r\n\r\n", b"\n\n@late\nACGTACGTACGTACGTACGTACGTACGTACGTACGT\n+\nII\n"])
+def test_fastq_blank_lines_open_no_record(chunk, tail):
+    """A text ending in a blank line (or holding one between records) has the records the oracle-side reader finds, no
+    extra empty one (A23): the record count, the filter and the per-record hit counts agree, with max_records equal to
+    the true count."""
+    genome = seqgen.markov(32, 5, 0.41, 30_000)
+    recs = [r for r in seqgen.reads(10, genome, 0, 60, 150, 0.01).reshape(60, 150)]
+    text = seqgen.fastq_text(recs, False, final_newline=False) + tail
+    n_want = len(fastx.parse(text, fastx.FASTQ)[1])
+    assert n_want == 60 + (tail.count(b"II") > 0)          # the grid-shifted tail yields one (empty) record more
+    for fmt in (0, fastx.FASTQ):
+        o = _check_insert(DEFAULT, 0, text, chunk, fmt=fmt)
+        o.close()
+    o = oracle.OracleSBF(num_bits=1 << 22, **DEFAULT)
+    o.insert_records(genome)
+    bases, offs = fastx.dense(text, fastx.FASTQ, with_pre=False)
+    _, want_counts, _ = o.query_records(bases, offs, threads=True)
+    with sbf.SuperBloomFilter(num_bits=1 << 22, **DEFAULT) as f:
+        d = torch.from_numpy(genome).cuda()
+        sbf.sbf_insert_seq(f.handle, d, d.numel())
+        if chunk:
+            sbf.sbf_set_host_chunk(f.handle, chunk)
+        hc = np.full(n_want, 0xFFFFFFFF, dtype=np.uint32)
+        n_rec, _ = sbf.sbf_query_fastx_host(f.handle, text, len(text), hc, n_want, fastx.FASTQ)   # capacity = true count
+        assert n_rec == n_want and np.array_equal(hc, want_counts)
+    o.close()
+
+
 def test_degenerate_texts():
     with sbf.SuperBloomFilter(num_bits=1 << 16, **DEFAULT) as f:
         for text in (b"", b"\n\n\n", b">only a header", b">h\n", b"@h\n\n+\n\n", b"ACGT", b">a\n>b\n>c\n"):

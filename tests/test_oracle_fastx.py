@@ -25,6 +25,19 @@ def test_fastq_literal():
     assert fastx.parse(b"@a\nAC\n+\nII")[1] == [b"AC"]
 
 
+def test_fastq_blank_lines_open_no_record():
+    """DESIGN.md A23: a line of index 0 mod 4 whose first byte is a line end still counts as a line but starts no record
+    (a text that ends in two newlines has no extra empty record)."""
+    assert fastx.parse(b"@a\nAC\n+\nII\n\n")[1] == [b"AC"]
+    assert fastx.parse(b"@a\nAC\n+\nII\n\n\n\n")[1] == [b"AC"]
+    assert fastx.parse(b"@a\r\nAC\r\n+\r\nII\r\n\r\n")[1] == [b"AC"]
+    assert fastx.dense(b"@a\nAC\n+\nII\n\n")[1].tolist() == [0, 2]
+    # a blank line BETWEEN records shifts the four-line grid (not valid FASTQ; the rule is only that both sides agree):
+    # line 4 is blank -> no start, line 5 "@b" is then a sequence line of record a, line 8 "II" starts a record whose
+    # sequence line (line 9) is empty
+    assert fastx.parse(b"@a\nAC\n+\nII\n\n@b\nGG\n+\nII\n")[1] == [b"AC@b", b""]
+
+
 def test_generators_round_trip():
     recs = [seqgen.uniform(1, 130), seqgen.uniform(2, 0), seqgen.uniform(3, 61), seqgen.uniform(4, 60)]
     for crlf in (False, True):
