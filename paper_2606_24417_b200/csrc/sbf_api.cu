@@ -268,6 +268,7 @@ int run_main(sbf *f, uint64_t total, uint32_t *bitmap, cudaStream_t st)
     if (f->entry) {
         CK((INSERT ? (f->tma_flush ? f->entry->insert_tma : f->entry->insert) : f->entry->query)(p, st));
     } else {
+        if (f->k > 32) return fail(SBF_ERR_UNSUPPORTED, "internal: naive_kernel packs a k-mer into one 64-bit word (k <= 32)");
         NaiveParams np;
         np.sp = p; np.k = f->k; np.m = f->m; np.s = f->s; np.H = f->H;
         uint64_t n32 = (total + 31) / 32 * 32;
@@ -453,7 +454,9 @@ sbf_t *sbf_create_ex(int k, int m, int s, int H, uint64_t num_bits, int alphabet
     f->k = k; f->m = m; f->s = s; f->H = H; f->P = P; f->device = dev;
     f->alphabet = alphabet; f->sym_bits = sym_bits; f->sym_bytes = alphabet == SBF_ALPHABET_DNA_TRIPLET ? 3 : 1;
     // DNA with 33 <= k <= 64 has specialised streaming instances too (folded wide windows, A21); without one: wide_tile_kernel
-    f->wide = alphabet != SBF_ALPHABET_DNA || (k > 32 && find_entry(k, m, s, H) == nullptr);
+    // (with 2^32 shards the instances are not used at all — see f->entry below — and naive_kernel packs a k-mer into one
+    // 64-bit word, so k > 32 must take the wide kernel there as well)
+    f->wide = alphabet != SBF_ALPHABET_DNA || (k > 32 && (P >= 32 || find_entry(k, m, s, H) == nullptr));
     f->num_shards = shards;
     f->host_chunk = kHostChunkDefault;
     f->tma_flush = shards * 32 >= kTmaFlushMinBytes;
