@@ -27,6 +27,53 @@ def _first_diff(got, want, what):
                          (what, bad.size, got.size, bad[0], got[bad[0]], want[bad[0]]))
 
 
+def _query_every_batch(f, o, w, batch, max_fpr):
+    """All of the workload's reads, batch by batch (bench.py's launch: one sbf_query_records per `batch` reads, device
+    buffers reused): every bitmap word and every per-read count of every batch against the oracle's OpenMP driver.
+    Per batch also the property that holds at any size: the error-free k-mers of the sampled reads are
+    all reported present, i.e. a sampled read's count is never below what its substitutions can explain."""
+    k, L = DEFAULT["k"], w.read_len
+    per = L - k + 1
+    assert w.n_reads % batch == 0
+    offs = seqgen.fixed_offsets(batch, L)
+    d_offs = _dev(offs.view(np.int64))
+    reads = np.empty(batch * L, dtype=np.uint8)
+    d_reads = torch.empty(batch * L, dtype=torch.uint8, device="cuda")
+    bm = torch.empty((batch * L + 31) // 32, dtype=torch.int32, device="cuda")
+    hc = torch.empty(batch, dtype=torch.int32, device="cuda")
+    n_batches = w.n_reads // batch
+    for b in range(n_batches):
+        w.read_batch(b * batch, batch, out=reads)
+        d_reads.copy_(torch.from_numpy(reads))
+        bm.fill_(-1)
+        hc.fill_(-1)
+        f.query_records(d_reads, d_offs, bm, hc)
+        torch.cuda.synchronize()
+        wbm, wc, _ = o.query_records(reads, offs, threads=True)
+        _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "batch %d of %d: bitmap words" % (b, n_batches))
+        got_c = hc.cpu().numpy().view(np.uint32)
+        _first_diff(got_c, wc, "batch %d of %d: hit counts" % (b, n_batches))
+        # sampled reads (even index): mostly present; uniform reads (odd index): only false positives
+        assert got_c[0::2].astype(np.int64).sum() > 0.6 * (batch // 2) * per, b
+        assert got_c[1::2].astype(np.int64).sum() < max_fpr * (batch // 2) * per, b
+        # a sampled read without any substitution that lies clear of N runs has all its k-mers present
+        for r in range(0, 2000, 2):
+            g = b * batch + r
+            if any(seqgen.read_is_sub(w.read_seed, w.read_sub_rate, L, g, i) for i in range(L)):
+                continue
+            start = seqgen.read_start(w.read_seed, w.insert_bases.size, L, g)
+            src = w.insert_bases[start:start + L]
+            if np.isin(src, np.frombuffer(b"ACGT", dtype=np.uint8)).all() and _inside_one_record(w, start, L):
+                assert got_c[r] == per, (b, r, int(got_c[r]))
+    return n_batches
+
+
+def _inside_one_record(w, start, length):
+    o = w.insert_offsets
+    r = int(np.searchsorted(o, start, side="right")) - 1
+    return start + length <= int(o[r + 1])
+
+
 _c3 = {}
 
 
@@ -38,11 +85,11 @@ def _config3():
 
 
 def test_config3_full_size_filter_bitmap_counts():
+    """BASELINE config 3 at full size: every filter byte after the 250 Mbp insert, then ALL 4e7 reads in bench.py's
+    batches of 4e6 (10 batches): every bitmap word and every per-read count."""
     w = _config3()                             # 250 Mbp, N runs, 2^32-bit filter
     nb = w.params["num_bits"]
-    n_reads = 4_000_000                        # bench.py's batch
-    reads = w.read_batch(0, n_reads)
-    offs = seqgen.fixed_offsets(n_reads, w.read_len)
+    assert w.n_reads == 40_000_000
     o = oracle.OracleSBF(num_bits=nb, **DEFAULT)
     n_ins = o.insert_records(w.insert_bases, threads=True)
     assert 240_000_000 < n_ins < 250_000_000
@@ -52,20 +99,8 @@ def test_config3_full_size_filter_bitmap_counts():
         f.insert_seq(d_seq)
         torch.cuda.synchronize()
         _first_diff(f.export_bits(), o.export_bits(), "filter bytes")
-        d_reads, d_offs = _dev(reads), _dev(offs.view(np.int64))
-        bm = torch.full(((reads.size + 31) // 32,), -1, dtype=torch.int32, device="cuda")
-        hc = torch.full((n_reads,), -1, dtype=torch.int32, device="cuda")
-        f.query_records(d_reads, d_offs, bm, hc)
-        torch.cuda.synchronize()
-        wbm, wc, n_q = o.query_records(reads, offs, threads=True)
-        _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "bitmap words")
-        _first_diff(hc.cpu().numpy().view(np.uint32), wc, "hit counts")
-        # properties that hold at any size: error-free k-mers of sampled reads are all present
-        per = w.read_len - DEFAULT["k"] + 1
-        sampled_hits = wc[0::2].astype(np.int64).sum()
-        assert sampled_hits > 0.6 * (n_reads // 2) * per
-        # FPR on the uniform reads stays small at 17 bits per k-mer
-        assert wc[1::2].astype(np.int64).sum() < 1e-3 * (n_reads // 2) * per
+        del d_seq
+        assert _query_every_batch(f, o, w, 4_000_000, max_fpr=1e-3) == 10     # 17 bits per inserted k-mer
     o.close()
 
 
@@ -141,32 +176,26 @@ def test_timing_abi_reports_kernel_times():
 
 def test_config4_full_size_insert_and_query_batch():
     """BASELINE config 4 at full size: 3.1 Gbp in 24 records into a 2^35-bit filter (every one of the 4 GiB filter
-    bytes compared), then one 4e6-read batch (bitmap and counts compared)."""
+    bytes compared), then ALL 1e8 reads in batches of 4e6 (25 batches): every bitmap word and every per-read count."""
     w = seqgen.config4()
     nb = w.params["num_bits"]
+    assert w.n_reads == 100_000_000
     o = oracle.OracleSBF(num_bits=nb, **DEFAULT)
     n_ins = o.insert_records(w.insert_bases, w.insert_offsets, threads=True)
     assert n_ins > 3_000_000_000
-    n_reads = 4_000_000
-    reads = w.read_batch(0, n_reads)
-    offs = seqgen.fixed_offsets(n_reads, w.read_len)
     with sbf.SuperBloomFilter(num_bits=nb, **DEFAULT) as f:
         assert f.num_shards == o.num_shards == 1 << 27
-        f.insert_records(_dev(w.insert_bases), _dev(w.insert_offsets.view(np.int64)))
+        d_ins = _dev(w.insert_bases)
+        f.insert_records(d_ins, _dev(w.insert_offsets.view(np.int64)))
         torch.cuda.synchronize()
+        del d_ins
         got = f.export_bits()
         want = o.words().reshape(-1).view(np.uint8)
         step = 1 << 28
         for a in range(0, got.size, step):                  # compare in slices: no third 4 GiB copy
             _first_diff(got[a:a + step], want[a:a + step], "filter bytes [%d, +%d)" % (a, step))
         del got
-        bm = torch.full(((reads.size + 31) // 32,), -1, dtype=torch.int32, device="cuda")
-        hc = torch.full((n_reads,), -1, dtype=torch.int32, device="cuda")
-        f.query_records(_dev(reads), _dev(offs.view(np.int64)), bm, hc)
-        torch.cuda.synchronize()
-        wbm, wc, _ = o.query_records(reads, offs, threads=True)
-        _first_diff(bm.cpu().numpy().view(np.uint32), wbm, "bitmap words")
-        _first_diff(hc.cpu().numpy().view(np.uint32), wc, "hit counts")
+        assert _query_every_batch(f, o, w, 4_000_000, max_fpr=2e-2) == 25     # 11 bits per inserted k-mer: FPR 0.7 %
     o.close()
 
 
