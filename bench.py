@@ -497,10 +497,13 @@ def run_cuda(args):
             r["binds_busy"] = busy[r["binds"]]
         dom = "query_kernel" if qk * 1.0 >= ik else "insert_kernel"
         traffic, traffic_src = load_traffic(dom)
-        roofline = {"bound": "alu", "kernel": dom, "achieved": roof[dom]["achieved"], "peak": roof[dom]["peak"],
-                    "unit": "Tiop/s", "frac": roof[dom]["frac"], "traffic": traffic, "traffic_source": traffic_src,
-                    "peak_source": roof[dom]["peak_source"], "binds": roof[dom]["binds"],
-                    "hbm": roof[dom]["hbm"]}
+        roofline = top_roofline(roof[dom], dom, traffic, traffic_src)
+        # the one driver-timed number against a roofline of its own: both fused kernels at the limit that binds them
+        # plus the streamed bytes of the passes around them (pack: 1 B/base in, 0.375 B/base out, + the result bitmap
+        # zeroed in passing for the reads; clear: the filter written once) at the measured HBM rate
+        roofline["step"] = step_roofline(roof, total_ms / args.steps,
+                                         pack_bytes=d_seq.numel() * 1.375 + n_read_bases * 1.5,
+                                         clear_bytes=num_bits / 8.0, hbm_gbs=hbm_gbs)
         line = {
             "metric": METRIC,
             "value": value, "unit": "G k-mers/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -639,6 +642,45 @@ def measure_ceilings(sbf, filter_bytes, gpu_index, sm_max_mhz):
             if nv.h is not None else "NVML unavailable: sm_max_mhz assumed",
             "pipe_warp_inst_per_clk_per_smsp": per_clk,
             "random_sector_g_per_s": rnd, "random_sector_array_bytes": int(min(filter_bytes, 8 << 30))}
+
+
+def top_roofline(r, kernel, traffic, traffic_src):
+    """The line's `roofline` object for the dominant kernel `r` (an entry of `rooflines`): quoted against the measured
+    limit that BINDS the kernel (`binds`: the busiest of the instruction limits, the random-sector rate and the streamed
+    HBM bytes), with the instruction roofline — both counts, the restated one of DESIGN.md §6 and SURVEY.md §8(d)'s
+    planning figure — beside it under "alu"."""
+    alu = {"achieved": r["achieved"], "peak": r["peak"], "unit": "Tiop/s", "frac": r["frac"],
+           "frac_with_survey_count": r.get("frac_with_survey_count"),
+           "ops_per_kmer": sum(r["algorithmic_ops_per_kmer"].values()),
+           "survey_ops_per_kmer": r.get("survey_planning_ops_per_kmer"), "peak_source": r["peak_source"]}
+    binds = r["binds"]
+    if binds == "random_sector":
+        rs = r["random_sector"]
+        out = {"bound": "hbm", "limit": "random 32-byte sector accesses: DRAM transactions, not bytes, bind (profiles/ceilings_ncu_r02.md)",
+               "achieved": rs["achieved_g_per_s"] * 32.0, "peak": rs["ceiling_g_per_s"] * 32.0, "unit": "GB/s",
+               "frac": rs["frac"], "peak_source": "measured in this run: %s, x 32 B" % rs["ceiling"]}
+    elif binds == "hbm_bytes":
+        out = {"bound": "hbm", "limit": "streamed bytes", "achieved": r["hbm"]["achieved"], "peak": r["hbm"]["peak"],
+               "unit": "GB/s", "frac": r["hbm"]["frac"], "peak_source": r["hbm"]["peak_source"]}
+    else:  # an instruction limit: the algorithmic instruction roofline is the fraction
+        out = {"bound": "alu", "limit": binds, "achieved": r["achieved"], "peak": r["peak"], "unit": "Tiop/s",
+               "frac": r["frac"], "peak_source": r["peak_source"]}
+    out.update({"kernel": kernel, "binds": binds, "binds_busy": r["binds_busy"], "traffic": traffic,
+                "traffic_source": traffic_src, "alu": alu, "random_sector": r["random_sector"], "hbm_streaming": r["hbm"]})
+    return out
+
+
+def step_roofline(roof, ms_per_step, pack_bytes, clear_bytes, hbm_gbs):
+    """Shortest time one step could take on this box: each fused kernel at the measured limit that binds it
+    (its time x the busy fraction of that limit) + the streamed bytes of pack and clear at the HBM rate."""
+    t_i = roof["insert_kernel"]["ms"] * min(1.0, roof["insert_kernel"]["binds_busy"])
+    t_q = roof["query_kernel"]["ms"] * min(1.0, roof["query_kernel"]["binds_busy"])
+    t_s = (pack_bytes + clear_bytes) / (hbm_gbs * 1e9) * 1e3
+    return {"roofline_ms": t_i + t_q + t_s, "ms_per_step": ms_per_step, "frac": (t_i + t_q + t_s) / ms_per_step,
+            "parts_ms": {"insert_kernel_at_%s" % roof["insert_kernel"]["binds"]: t_i,
+                         "query_kernel_at_%s" % roof["query_kernel"]["binds"]: t_q,
+                         "pack_and_clear_bytes_at_hbm": t_s},
+            "timed": "sbf_clear + sbf_insert_seq/_records + sbf_query_records of one read batch (pack, fused kernels, counts)"}
 
 
 def alu_roofline(ops, n_units, ms, ceil, clock_mhz, executed, survey_ops=None):

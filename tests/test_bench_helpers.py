@@ -77,3 +77,34 @@ def test_static_profile_tables_load():
     assert rows and {"kernel", "dram_bytes_per_launch", "source"} <= set(rows[0])
     t, src = bench.load_traffic("query_kernel")
     assert t > 0 and "ncu" in src
+
+
+def _kernel_entry(frac_alu, frac_rs, frac_hbm, ms):
+    return {"achieved": 10.0 * frac_alu, "peak": 10.0, "frac": frac_alu, "frac_with_survey_count": frac_alu * 1.4, "ms": ms,
+            "algorithmic_ops_per_kmer": {"alu": 39.0, "fma": 4.0, "wide": 3.0}, "survey_planning_ops_per_kmer": 63.0,
+            "peak_source": "x", "binds": max((("alu_pipe", frac_alu), ("random_sector", frac_rs), ("hbm_bytes", frac_hbm)),
+                                              key=lambda kv: kv[1])[0],
+            "binds_busy": max(frac_alu, frac_rs, frac_hbm),
+            "random_sector": {"achieved_g_per_s": 48.0 * frac_rs, "ceiling_g_per_s": 48.0, "frac": frac_rs, "ceiling": "loads"},
+            "hbm": {"achieved": 6000.0 * frac_hbm, "peak": 6000.0, "unit": "GB/s", "frac": frac_hbm, "peak_source": "m"}}
+
+
+def test_top_roofline_quotes_the_binding_limit():
+    """roofline.bound / frac follow the limit that binds; the instruction fractions (both counts) stay beside it."""
+    r = bench.top_roofline(_kernel_entry(0.80, 0.92, 0.30, 1.5), "query_kernel", 123, "src")
+    assert r["bound"] == "hbm" and r["binds"] == "random_sector" and r["unit"] == "GB/s"
+    assert abs(r["frac"] - 0.92) < 1e-12 and abs(r["achieved"] / r["peak"] - r["frac"]) < 1e-12
+    assert r["alu"]["frac"] == 0.80 and r["alu"]["ops_per_kmer"] == 46.0 and r["alu"]["survey_ops_per_kmer"] == 63.0
+    assert r["traffic"] == 123 and r["kernel"] == "query_kernel"
+    r = bench.top_roofline(_kernel_entry(0.85, 0.50, 0.30, 1.5), "query_kernel", None, None)
+    assert r["bound"] == "alu" and r["frac"] == 0.85 and r["unit"] == "Tiop/s"
+    r = bench.top_roofline(_kernel_entry(0.2, 0.3, 0.7, 1.5), "insert_kernel", None, None)
+    assert r["bound"] == "hbm" and r["limit"] == "streamed bytes" and r["frac"] == 0.7
+
+
+def test_step_roofline_adds_up():
+    roof = {"insert_kernel": _kernel_entry(0.7, 0.97, 0.3, 1.2), "query_kernel": _kernel_entry(0.8, 0.9, 0.3, 1.4)}
+    s = bench.step_roofline(roof, 2.9, pack_bytes=6.0e8, clear_bytes=4.0e8, hbm_gbs=5000.0)
+    want = 1.2 * 0.97 + 1.4 * 0.9 + 1.0e9 / 5.0e12 * 1e3
+    assert abs(s["roofline_ms"] - want) < 1e-9 and abs(s["frac"] - want / 2.9) < 1e-9
+    assert abs(sum(s["parts_ms"].values()) - s["roofline_ms"]) < 1e-9
