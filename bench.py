@@ -636,7 +636,7 @@ def measure_ceilings(sbf, filter_bytes, gpu_index, sm_max_mhz):
             rnd[nm] = sbf.sbf_ceiling_random_sector(mode, min(filter_bytes, 8 << 30))
         except Exception:  # noqa: BLE001 - a ceiling that cannot be measured is reported as such
             rnd[nm] = None
-    return {"source": "measured in this run (sbf_ceiling_pipe_rate / sbf_ceiling_random_sector, include/sbf.h)",
+    return {"source": "measured in this run (sbf_ceiling_pipe_rate / sbf_ceiling_random_sector, include/sbf_bench.h, libsbf_bench_b200.so)",
             "pipe_g_warp_inst_per_s_per_smsp": per_s, "sm_clock_mhz_during_pipe_runs": clocks,
             "sm_clock_source": "NVML nvmlDeviceGetClockInfo(SM) sampled every 4 ms during each run"
             if nv.h is not None else "NVML unavailable: sm_max_mhz assumed",

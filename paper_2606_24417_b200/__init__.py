@@ -18,7 +18,9 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsbf_b200.so")
+BENCH_LIB_PATH = os.path.join(_HERE, "libsbf_bench_b200.so")
 _lib = None
+_bench_lib = None
 
 SBF_OK = 0
 SBF_ERR_INVALID_ARG = -1
@@ -62,11 +64,14 @@ ABI = {
     "sbf_set_host_chunk": (_i32, [_p, _u64]),
     "sbf_set_timing": (_i32, [_p, _i32]),
     "sbf_get_timing": (_i32, [_p, _p]),
-    "sbf_debug_last_packed": (_i32, [_p, _p, _p, _u64]),
+}
+# every symbol include/sbf_bench.h declares (libsbf_bench_b200.so: measurement and test hooks, not the product boundary)
+BENCH_ABI = {
     "sbf_ceiling_pipe_modes": (_i32, []),
     "sbf_ceiling_pipe_mode_name": (_cp, [_i32]),
     "sbf_ceiling_pipe_rate": (_i32, [_i32, _i32, _p, _p]),
     "sbf_ceiling_random_sector": (_i32, [_i32, _u64, _p]),
+    "sbf_bench_pack": (_i32, [_p, _u64, _i32, _p, _p, _u64]),
 }
 
 
@@ -97,6 +102,28 @@ def load_library(build_if_missing: bool = True):
         fn.argtypes = args
     _lib = L
     return L
+
+
+def load_bench_library():
+    """dlopen libsbf_bench_b200.so (include/sbf_bench.h) — bench.py, the ceilings CLI and the tests only."""
+    global _bench_lib
+    if _bench_lib is not None:
+        return _bench_lib
+    load_library()                          # runs the incremental build of both libraries
+    if not os.path.exists(BENCH_LIB_PATH):
+        raise SBFError(SBF_ERR_UNSUPPORTED, "libsbf_bench_b200.so not built (python -m paper_2606_24417_b200.build)")
+    L = ctypes.CDLL(BENCH_LIB_PATH)
+    for name, (res, args) in BENCH_ABI.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    _bench_lib = L
+    return L
+
+
+def _check_bench(rc: int, what: str):
+    if rc != SBF_OK:
+        raise SBFError(rc, "%s failed (libsbf_bench_b200.so returns codes only)" % what)
 
 
 def _check(rc: int):
@@ -298,28 +325,29 @@ def sbf_get_timing(h):
     return float(ms[0]), float(ms[1]), float(ms[2])
 
 
-def sbf_ceiling_pipe_modes() -> int: return int(load_library().sbf_ceiling_pipe_modes())
-def sbf_ceiling_pipe_mode_name(mode: int) -> str: return load_library().sbf_ceiling_pipe_mode_name(mode).decode()
+def sbf_ceiling_pipe_modes() -> int: return int(load_bench_library().sbf_ceiling_pipe_modes())
+def sbf_ceiling_pipe_mode_name(mode: int) -> str: return load_bench_library().sbf_ceiling_pipe_mode_name(mode).decode()
 
 
 def sbf_ceiling_pipe_rate(mode: int, iters: int = 2048):
     """(1e9 warp instructions per second per SM sub-partition, clock64() rate in MHz) of one instruction mix."""
     r, c = ctypes.c_double(0), ctypes.c_double(0)
-    _check(load_library().sbf_ceiling_pipe_rate(mode, iters, ctypes.addressof(r), ctypes.addressof(c)))
+    _check_bench(load_bench_library().sbf_ceiling_pipe_rate(mode, iters, ctypes.addressof(r), ctypes.addressof(c)), "sbf_ceiling_pipe_rate")
     return float(r.value), float(c.value)
 
 
 def sbf_ceiling_random_sector(mode: int, array_bytes: int) -> float:
     """Random 32-byte-sector accesses per second (1e9/s) over array_bytes."""
     g = ctypes.c_double(0)
-    _check(load_library().sbf_ceiling_random_sector(mode, array_bytes, ctypes.addressof(g)))
+    _check_bench(load_bench_library().sbf_ceiling_random_sector(mode, array_bytes, ctypes.addressof(g)), "sbf_ceiling_random_sector")
     return float(g.value)
 
 
-def sbf_debug_last_packed(h, n_words: int):
+def sbf_bench_pack(d_seq, length: int, k: int, n_words: int):
+    """(packed 2-bit words, validity masks) of the first n_words 16-symbol words, as pack_kernel writes them."""
     w = np.empty(n_words, dtype=np.uint32)
     g = np.empty(n_words, dtype=np.uint16)
-    _check(load_library().sbf_debug_last_packed(h, w.ctypes.data, g.ctypes.data, n_words))
+    _check_bench(load_bench_library().sbf_bench_pack(_dptr(d_seq), length, k, w.ctypes.data, g.ctypes.data, n_words), "sbf_bench_pack")
     return w, g
 
 

@@ -1,4 +1,6 @@
-"""Build the CUDA library in-tree: csrc/*.cu -> paper_2606_24417_b200/libsbf_b200.so (sm_100a).
+"""Build the CUDA libraries in-tree (sm_100a):
+  csrc/*.cu except sbf_bench*.cu -> paper_2606_24417_b200/libsbf_b200.so        the product (include/sbf.h)
+  csrc/sbf_bench*.cu             -> paper_2606_24417_b200/libsbf_bench_b200.so  measurement / test hooks (include/sbf_bench.h)
 
 nvcc cross-compiles without a GPU.  The translation units are compiled in parallel; an object is
 rebuilt only when its source or a header is newer.  `python -m paper_2606_24417_b200.build [--force]`.
@@ -16,6 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 OBJDIR = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsbf_b200.so")
+BENCH_LIB = os.path.join(HERE, "libsbf_bench_b200.so")
 
 SWEEP_S = (24, 26, 28, 30, 31)   # BASELINE.json configs[4]
 SWEEP_M = (12, 14, 16, 18, 20)
@@ -40,9 +43,21 @@ def _headers():
         glob.glob(os.path.join(INCLUDE, "*.h"))
 
 
+def _is_bench(src: str) -> bool:
+    return os.path.basename(src).startswith("sbf_bench")
+
+
 def build(force: bool = False, verbose: bool = False, extra_flags=(), lib: str = LIB, objdir: str = OBJDIR) -> str:
-    """extra_flags / lib / objdir: build a variant (-D switches) next to the product library."""
-    srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
+    """Both libraries; returns the product library's path.  extra_flags / lib / objdir: build a variant (-D switches) of
+    the product library next to it (the bench library is then left alone)."""
+    out = _build(False, force, verbose, extra_flags, lib, objdir)
+    if lib == LIB:
+        _build(True, force, verbose, (), BENCH_LIB, objdir)
+    return out
+
+
+def _build(bench: bool, force: bool, verbose: bool, extra_flags, lib: str, objdir: str) -> str:
+    srcs = sorted(s for s in glob.glob(os.path.join(CSRC, "*.cu")) if _is_bench(s) == bench)
     if not srcs:
         raise RuntimeError("no CUDA sources under %s" % CSRC)
     hdr_time = max(os.path.getmtime(h) for h in _headers())

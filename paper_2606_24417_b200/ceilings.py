@@ -4,7 +4,7 @@
 
 Issue rates of one SM sub-partition by instruction mix (1e9 warp instructions per second, counted in SASS) and random
 32-byte-sector access rates over an array of `--bytes` (1e9 accesses per second), through the C ABI
-(sbf_ceiling_pipe_rate / sbf_ceiling_random_sector, include/sbf.h).  bench.py calls the same entry points in its own
+(sbf_ceiling_pipe_rate / sbf_ceiling_random_sector, include/sbf_bench.h, libsbf_bench_b200.so).  bench.py calls the same entry points in its own
 run; this front end exists so that the micro-benchmarks can be profiled on their own (profiles/ceilings_ncu_r02.md).
 """
 from __future__ import annotations

@@ -476,7 +476,9 @@ sbf_t *sbf_create_ex(int k, int m, int s, int H, uint64_t num_bits, int alphabet
     cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev);
     cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev);
     uint64_t bytes = shards * 32;
-    if (max_persist > 0 && bytes <= (uint64_t)max_persist && bytes <= (uint64_t)max_window && bytes >= (1u << 20)) {
+    const char *l2_env = getenv("SBF_L2_WINDOW"); // "0": no persistence window and no device-wide limit change (A/B switch, profiles/l2_window_r03.md)
+    const bool l2_allowed = !(l2_env && l2_env[0] == '0');
+    if (l2_allowed && max_persist > 0 && bytes <= (uint64_t)max_persist && bytes <= (uint64_t)max_window && bytes >= (1u << 20)) {
         size_t cur = 0;
         cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize);
         if (cur < bytes) cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, (size_t)max_persist);
@@ -690,16 +692,6 @@ int sbf_ipc_close_filter(uint64_t *d_ptr)
 {
     if (!d_ptr) return SBF_OK;
     CK(cudaIpcCloseMemHandle(d_ptr));
-    return SBF_OK;
-}
-
-int sbf_debug_last_packed(const sbf_t *f, uint32_t *h_words, uint16_t *h_mask, uint64_t n_words)
-{
-    if (!f || !h_words || !h_mask) return fail(SBF_ERR_INVALID_ARG, "sbf_debug_last_packed: NULL argument");
-    if (n_words > f->last_words) return fail(SBF_ERR_INVALID_ARG, "sbf_debug_last_packed: more words than the last batch");
-    CK(cudaDeviceSynchronize());
-    CK(cudaMemcpy(h_words, f->packed, n_words * sizeof(uint32_t), cudaMemcpyDeviceToHost));
-    CK(cudaMemcpy(h_mask, f->gmask, n_words * sizeof(uint16_t), cudaMemcpyDeviceToHost));
     return SBF_OK;
 }
 

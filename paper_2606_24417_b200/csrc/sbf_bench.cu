@@ -1,4 +1,6 @@
-// sbf_ceilings.cu — measured ceilings of the device the rooflines are quoted against ("measure ...
+// sbf_bench.cu — libsbf_bench_b200.so (include/sbf_bench.h): measurement and test hooks kept OUT of the product library.
+//
+// Measured ceilings of the device the rooflines are quoted against ("measure ...
 // before quoting a denominator").  Not part of the hot path: bench.py calls these two entry points in the same run,
 // on the same box and clocks as the kernels it times, and writes the results into its JSON line.
 //
@@ -11,7 +13,10 @@
 //                              not tick at the SM clock (it gave 1.58 warp instructions per "cycle" per SMSP).
 //   sbf_ceiling_random_sector  random 32-byte-sector accesses per second over an array of a given size, with exactly
 //                              the access the fused kernels make (4 x RED.OR.B64 per sector; 2 x 16-byte cp.async; ...)
-#include "../../include/sbf.h"
+#include "../../include/sbf_bench.h"
+
+#define SBF_DEFINE_AUX_KERNELS // the copy of pack_kernel that sbf_bench_pack launches
+#include "sbf_device.cuh"
 
 #include <cstdint>
 #include <cstdio>
@@ -273,6 +278,33 @@ int sbf_ceiling_random_sector(int mode, uint64_t array_bytes, double *g_accesses
     if (err != cudaSuccess) return SBF_ERR_CUDA;
     *g_accesses_per_s = (double)blocks * kRandTPB * per_thread / (best * 1e-3) / 1e9;
     return SBF_OK;
+}
+
+
+// a1 on its own (tests/test_gpu_parity.py::test_pack_kernel_words_and_mask): pack_kernel launched exactly as the
+// insert / query calls of the product library launch it, its two outputs copied to the host.
+int sbf_bench_pack(const char *d_seq, uint64_t len, int k, uint32_t *h_words, uint16_t *h_mask, uint64_t n_words)
+{
+    if ((!d_seq && len) || !h_words || !h_mask || k < 1 || k > 64) return SBF_ERR_INVALID_ARG;
+    const uint64_t nw = (len + 15) / 16 + sbfk::kPadWords;
+    if (n_words > nw) return SBF_ERR_INVALID_ARG;
+    uint32_t *packed = nullptr;
+    uint16_t *vmask = nullptr;
+    if (cudaMalloc(&packed, nw * sizeof(uint32_t)) != cudaSuccess || cudaMalloc(&vmask, nw * sizeof(uint16_t) + 8) != cudaSuccess) {
+        cudaFree(packed);
+        cudaGetLastError();
+        return SBF_ERR_NOMEM;
+    }
+    const unsigned blocks = (unsigned)(((nw + 1) / 2 + 255) / 256);
+    const int aligned = ((reinterpret_cast<uintptr_t>(d_seq) & 15) == 0) ? 1 : 0;
+    sbfk::pack_kernel<<<blocks, 256>>>(reinterpret_cast<const uint8_t *>(d_seq), len, packed, vmask, nw, k, aligned, nullptr,
+                                       (len + 31) / 32, nullptr);
+    cudaError_t err = cudaGetLastError();
+    if (err == cudaSuccess) err = cudaMemcpy(h_words, packed, n_words * sizeof(uint32_t), cudaMemcpyDeviceToHost);
+    if (err == cudaSuccess) err = cudaMemcpy(h_mask, vmask, n_words * sizeof(uint16_t), cudaMemcpyDeviceToHost);
+    cudaFree(packed);
+    cudaFree(vmask);
+    return err == cudaSuccess ? SBF_OK : SBF_ERR_CUDA;
 }
 
 } // extern "C"

@@ -11,8 +11,8 @@ import paper_2606_24417_b200 as sbf
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def _declared_symbols():
-    text = open(os.path.join(ROOT, "include", "sbf.h")).read()
+def _declared_symbols(header="sbf.h"):
+    text = open(os.path.join(ROOT, "include", header)).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(sbf_[a-z0-9_]+)\s*\(", text)))
 
@@ -32,8 +32,23 @@ def test_header_symbols_are_exported_and_bound():
             assert callable(getattr(sbf, n)), n
 
 
+def test_bench_header_lives_in_its_own_library():
+    """include/sbf_bench.h (ceiling micro-benchmarks, pack test hook) is exported by libsbf_bench_b200.so only: the
+    product library carries none of it, and the product header declares none of it."""
+    B = sbf.load_bench_library()
+    L = sbf.load_library()
+    names = _declared_symbols("sbf_bench.h")
+    assert names == sorted(sbf.BENCH_ABI) and len(names) == 5
+    for n in names:
+        assert hasattr(B, n), "libsbf_bench_b200.so does not export %s" % n
+        assert not hasattr(L, n), "the product library exports the bench symbol %s" % n
+        assert n not in _declared_symbols("sbf.h")
+        assert callable(getattr(sbf, n))
+    assert not hasattr(L, "sbf_debug_last_packed")
+
+
 def test_header_has_no_torch_or_cuda_types():
-    text = open(os.path.join(ROOT, "include", "sbf.h")).read()
+    text = open(os.path.join(ROOT, "include", "sbf.h")).read() + open(os.path.join(ROOT, "include", "sbf_bench.h")).read()
     code = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
     assert "torch" not in code and "at::" not in code and "cuda_runtime" not in code
     assert 'extern "C"' in code

@@ -26,7 +26,7 @@ def _histograms():
     if not os.path.exists(cuobjdump):
         pytest.skip("cuobjdump not available")
     B.build()
-    obj = os.path.join(B.OBJDIR, "sbf_ceilings.o")
+    obj = os.path.join(B.OBJDIR, "sbf_bench.o")
     if not os.path.exists(obj):  # a shipped library without its objects (build() had nothing to do)
         B.build(force=True)
     sass = subprocess.run([cuobjdump, "-sass", obj], stdout=subprocess.PIPE, text=True, check=True).stdout

@@ -341,10 +341,8 @@ def test_pack_kernel_words_and_mask():
     seq[rng.integers(0, seq.size, 60)] = ord("N")
     seq[100:110] = np.frombuffer(b"acgtacgtXa", dtype=np.uint8)
     k = 31
-    with sbf.SuperBloomFilter(num_bits=1 << 14, **DEFAULT) as f:
-        gpu_insert(f, seq)
-        nw = (seq.size + 15) // 16
-        words, mask = sbf.sbf_debug_last_packed(f.handle, nw)
+    nw = (seq.size + 15) // 16
+    words, mask = sbf.sbf_bench_pack(dev(seq), seq.size, k, nw)      # pack_kernel as the insert / query calls launch it
     code = np.full(256, -1, dtype=np.int64)
     for ch, v in zip(b"ACGTacgt", [0, 1, 2, 3] * 2):
         code[ch] = v
