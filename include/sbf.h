@@ -58,9 +58,10 @@ typedef enum sbf_status {
  *   per shard, 32 bytes per shard, 32-byte aligned (one L2 sector per shard).
  *   (k,m,s,H) combinations compiled as specialised streaming kernels run those; every
  *   other legal combination runs a runtime-parameter CUDA kernel (same bits, slower).
- *   Side effect on the DEVICE (not only this handle): when the filter is small enough to be kept in L2 (a7), the
- *   call raises cudaLimitPersistingL2CacheSize to the device maximum if it is lower, and every later call on this
- *   handle sets an access-policy window for the filter on the stream it is given.
+ *   No device-wide side effects.  Only when the environment sets SBF_L2_WINDOW=1 and the filter fits the persisting L2
+ *   carve-out (a7) does the call raise cudaLimitPersistingL2CacheSize (a DEVICE-wide limit) and later calls on the
+ *   handle set an access-policy window for the filter on the stream they are given; measured on config 2 the window
+ *   changes neither kernel times nor L2 hit rates (profiles/l2_window_r03.md), hence off by default.
  *   Returns NULL on error.
  */
 sbf_t *sbf_create(int k, int m, int s, int H, uint64_t num_bits);

@@ -476,8 +476,10 @@ sbf_t *sbf_create_ex(int k, int m, int s, int H, uint64_t num_bits, int alphabet
     cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, dev);
     cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, dev);
     uint64_t bytes = shards * 32;
-    const char *l2_env = getenv("SBF_L2_WINDOW"); // "0": no persistence window and no device-wide limit change (A/B switch, profiles/l2_window_r03.md)
-    const bool l2_allowed = !(l2_env && l2_env[0] == '0');
+    // opt-in since round 3 (SBF_L2_WINDOW=1): measured to buy nothing on config 2 (profiles/l2_window_r03.md), and it is the
+    // only device-wide side effect sbf_create had
+    const char *l2_env = getenv("SBF_L2_WINDOW");
+    const bool l2_allowed = l2_env && l2_env[0] == '1';
     if (l2_allowed && max_persist > 0 && bytes <= (uint64_t)max_persist && bytes <= (uint64_t)max_window && bytes >= (1u << 20)) {
         size_t cur = 0;
         cudaDeviceGetLimit(&cur, cudaLimitPersistingL2CacheSize);
