@@ -164,7 +164,8 @@ struct sbf {
     uint16_t *gmask;
     uint64_t cap_words;       // allocated words in packed / gmask
     uint64_t last_words;      // words written by the last pack
-    uint32_t *d_flag;         // record-mode fallback flag of the last query (cleared by pack_kernel, raised by stream_rec_kernel)
+    uint32_t *d_flag;         // [0] record-mode fallback flag of the last query, [1] its long-record group counter (cleared by pack_kernel, raised by stream_rec_kernel)
+    uint2 *d_long;            // kLongCap (record, group) entries: the long records of the last record-mode query
     // L2 persistence window (a7)
     bool l2_window;
     cudaStream_t l2_stream_set;
@@ -257,6 +258,7 @@ StreamParams make_params(sbf *f, uint64_t total, uint32_t *bitmap)
     // short chunks for small batches, so that the grid still fills 148 SMs x 6 CTAs a few times over
     p.chunk_blocks = total >= (64ull << 20) ? 8 : total >= (16ull << 20) ? 4 : 2;
     p.offsets = nullptr; p.n_rec = 0; p.counts = nullptr; p.fallback = nullptr; p.rec_limit = 0;
+    p.long_groups = nullptr; p.long_cap = 0;
     return p;
 }
 
@@ -347,11 +349,15 @@ int run_count_records(const uint32_t *d_bitmap, const uint64_t *d_offsets, uint6
 }
 
 // Record mode (one thread per record, stream_rec_kernel) is tried for batches of short records: the host knows only
-// the MEAN length.  A thread that meets a record above kRecMaxLimit raises a device flag instead of walking it, and the
-// chunk-mode launches queued right behind (record-end marking, chunk kernel, count kernel) then redo the whole batch;
-// while the flag is clear they exit at once.  No host synchronisation either way.
+// the MEAN length.  A thread that meets a record above kRecMaxLimit lists it instead of walking it, and
+// stream_long_kernel, queued right behind, walks only the listed records chunk by chunk (it exits at once when the list
+// is empty).  Only when the list overflows (more than kLongCap groups) is the device flag raised, and the chunk-mode
+// launches queued behind (record-end marking, chunk kernel, count kernel) then redo the whole batch; while the flag is
+// clear they exit at once.  No host synchronisation either way.
 constexpr uint64_t kRecMeanLimit = 400; // symbols
 constexpr uint32_t kRecMaxLimit = 1024; // symbols
+// list of the long records' chunk groups (128 chunks of 128 positions each): 65536 groups = 1 Gi positions of long records
+constexpr uint32_t kLongCap = 65536;
 
 int run_query(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n_rec, uint64_t total, uint32_t *d_bitmap,
               uint32_t *d_counts, cudaStream_t st)
@@ -378,8 +384,13 @@ int run_query(sbf *f, const char *d_bases, const uint64_t *d_offsets, uint64_t n
     if (try_rec) {
         StreamParams p = make_params(f, total, d_bitmap);
         p.offsets = d_offsets; p.n_rec = n_rec; p.counts = d_counts; p.fallback = f->d_flag; p.rec_limit = kRecMaxLimit;
+        if (n_rec <= 0xFFFFFFFFull) { p.long_groups = f->d_long; p.long_cap = kLongCap; } // the list holds 32-bit record indices
         CK(f->entry->query_rec(p, st));
         g_launches++;
+        if (p.long_groups) {
+            CK(f->entry->query_long(p, st));
+            g_launches++;
+        }
         rc = mark(f, 2, st);
         if (rc) return rc;
         // the fallback behind record mode: all three exit at once unless a record was longer than kRecMaxLimit
@@ -464,10 +475,12 @@ sbf_t *sbf_create_ex(int k, int m, int s, int H, uint64_t num_bits, int alphabet
     e = cudaMalloc(&f->filter, shards * 32);
     if (e == cudaSuccess) e = cudaMemset(f->filter, 0, shards * 32);
     if (e == cudaSuccess) e = cudaMalloc(&f->d_flag, 256);
+    if (e == cudaSuccess) e = cudaMalloc(&f->d_long, (size_t)kLongCap * sizeof(uint2));
     if (e != cudaSuccess) {
         fail_cuda(e, "sbf_create: filter allocation");
         if (f->filter) cudaFree(f->filter);
         if (f->d_flag) cudaFree(f->d_flag);
+        if (f->d_long) cudaFree(f->d_long);
         delete f;
         return nullptr;
     }
@@ -501,6 +514,7 @@ void sbf_destroy(sbf_t *f)
     if (f->gmask) cudaFree(f->gmask);
     if (f->filter) cudaFree(f->filter);
     if (f->d_flag) cudaFree(f->d_flag);
+    if (f->d_long) cudaFree(f->d_long);
     cudaGetLastError();
     delete f;
 }
@@ -1213,6 +1227,7 @@ int sbf_query_seq_static(int k, int m, int s, int H, const uint64_t *d_filter, u
     p.n_bitmap_words = (len + 31) / 32;
     p.chunk_blocks = len >= (64ull << 20) ? 8 : len >= (16ull << 20) ? 4 : 2;
     p.offsets = nullptr; p.n_rec = 0; p.counts = nullptr; p.fallback = nullptr; p.rec_limit = 0;
+    p.long_groups = nullptr; p.long_cap = 0;
     if (entry) {
         CK(entry->query(p, st));
     } else {

@@ -12,6 +12,7 @@
 //   stream_kernel      a2-a6  the fused, thread-serial streaming insert / query kernel (chunk mode)
 //   stream_rec_kernel  a2-a6  the same query pipeline, one thread per short record (record mode)
 //                          query test: SlidingGather (byte-gather form, H <= 4) or SlidingOr (256-bit masks)
+//   stream_long_kernel a2-a6  the records of a record-mode batch that are too long for one thread, chunk by chunk
 //   naive_kernel       a2-a6  runtime-parameter one-k-mer-per-thread form of Alg. 1/2 (any legal k,m,s,H)
 //   wide_tile_kernel   a1-a6  the other alphabets and DNA k > 32 without an instance, from the ASCII bytes,
 //                          runtime parameters, a tile of 1024 byte positions per CTA through shared memory
@@ -103,7 +104,13 @@ struct StreamParams {
     uint32_t *fallback;      // device flag: record mode met a record above rec_limit -> the chunk kernels redo the batch
     uint32_t rec_limit;      // longest record one thread of stream_rec_kernel walks
     int chunk_blocks;        // chunk mode: 16-position blocks walked by one thread (2, 4 or 8: small batches use short chunks)
+    // record mode, records above rec_limit: stream_rec_kernel lists them as groups of kLongGroup chunks of kLongChunk
+    // positions, stream_long_kernel walks exactly those (the group counter is the word after `fallback`)
+    uint2 *long_groups;      // nullable: (record, group index inside the record)
+    uint32_t long_cap;       // entries long_groups holds; a batch that needs more falls back to the chunk kernels
 };
+constexpr uint32_t kLongChunk = 128; // positions per thread of stream_long_kernel, on the batch's 128-position grid
+constexpr uint32_t kLongGroup = SBF_STREAM_TPB; // chunks per CTA
 
 struct NaiveParams {
     StreamParams sp;
@@ -252,7 +259,8 @@ __device__ __forceinline__ void load32(const uint8_t *__restrict__ seq, uint64_t
 
 // bitmap_zero (nullable): the result bitmap of a record-mode query, whose word i covers exactly this thread's 32
 // symbols — zeroed here, in passing, because record mode ORs into the words two records share.
-// flag_zero (nullable): the record-mode fallback flag, cleared by the first thread.
+// flag_zero (nullable): the record-mode fallback flag and, in the next word, the long-record group counter, cleared by
+// the first thread.
 __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ seq, uint64_t len, uint32_t *__restrict__ packed,
                                                    uint16_t *__restrict__ vmask, uint64_t n_words_total, int k, int aligned16,
                                                    uint32_t *__restrict__ bitmap_zero, uint64_t n_bitmap_words,
@@ -261,7 +269,7 @@ __global__ void __launch_bounds__(256) pack_kernel(const uint8_t *__restrict__ s
     // thread i: symbols [32i, 32i+32) -> packed words 2i, 2i+1 (one 8-byte store) and their two mask words (one 4-byte store)
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const uint64_t b0 = i * 32;
-    if (i == 0 && flag_zero != nullptr) *flag_zero = 0;
+    if (i == 0 && flag_zero != nullptr) { flag_zero[0] = 0; flag_zero[1] = 0; } // fallback flag, long-record group counter
     uint32_t v[8];
     load32(seq, b0, len, aligned16, v);
     uint32_t word[2] = {0, 0}, inv = 0, bad = 0;
@@ -974,8 +982,10 @@ __global__ void __launch_bounds__(kStreamTPB, MODE != kModeQuery ? SBF_MINB_I : 
 // of the same registers.  The window is re-aligned to the record start with one funnel shift per
 // 16 symbols.  Output: pack_kernel zeroed the bitmap; words that lie wholly inside the record are
 // stored, the (at most two) words shared with neighbours are OR-ed in.
-// A record longer than rec_limit is not walked: the thread raises the fallback flag and the chunk
-// kernels, launched right after, redo the whole batch (they do nothing while the flag is clear).
+// A record longer than rec_limit is not walked here: the thread lists it for stream_long_kernel
+// (launched right after), which walks ONLY those records, chunk by chunk; the short records' results
+// stand.  Only a batch whose long records overflow the list raises the fallback flag, and the chunk
+// kernels, launched behind, then redo the whole batch (they do nothing while the flag is clear).
 // =============================================================================================
 template <int K, int M, int S, int H>
 #ifdef SBF_REC_MAXREG
@@ -990,6 +1000,19 @@ __global__ void __launch_bounds__(kRecTPB, SBF_MINB_R) stream_rec_kernel(const S
     if (r >= prm.n_rec) return;
     const uint64_t a = __ldg(prm.offsets + r), e = __ldg(prm.offsets + r + 1);
     if (e - a > (uint64_t)prm.rec_limit) {
+        // too long for one thread: hand the record to stream_long_kernel as groups of chunks on the batch's 128-position
+        // grid.  Only when the list cannot hold them (or there is none) does the flag go up and the chunk kernels redo
+        // the whole batch.
+        const uint64_t nch = ((e - 1) >> 7) - (a >> 7) + 1;
+        const uint64_t ngr = (nch + kLongGroup - 1) / kLongGroup;
+        if (prm.long_groups != nullptr && ngr <= (uint64_t)prm.long_cap) {
+            const uint32_t base = atomicAdd(prm.fallback + 1, (uint32_t)ngr);
+            if ((uint64_t)base + ngr <= (uint64_t)prm.long_cap) {
+                for (uint32_t j = 0; j < (uint32_t)ngr; ++j) prm.long_groups[base + j] = make_uint2((uint32_t)r, j);
+                if (prm.counts) prm.counts[r] = 0; // stream_long_kernel adds its chunks' hits
+                return;
+            }
+        }
         *prm.fallback = 1;
         return;
     }
@@ -1066,6 +1089,66 @@ __global__ void __launch_bounds__(kRecTPB, SBF_MINB_R) stream_rec_kernel(const S
     }
     if (rb) emit((uint32_t)rb);
     if (prm.counts) prm.counts[r] = cnt;
+}
+
+// =============================================================================================
+// a2-a6 fused, the LONG records of a record-mode batch: one CTA per listed group of kLongGroup chunks,
+// one thread per chunk of kLongChunk positions on the batch's 128-position grid — the chunk-mode
+// query pipeline (QueryLane, 8 blocks of 16), but the result bits are clipped to the record's k-mer
+// start positions [a, e-K+1) and OR-ed into the bitmap (pack_kernel zeroed it; the words at the two
+// ends are shared with the neighbouring records that stream_rec_kernel answered), and the hits are
+// added to the record's count.  The cost follows the long records' symbols only.
+// =============================================================================================
+template <int K, int M, int S, int H>
+__global__ void __launch_bounds__(kStreamTPB, 4) stream_long_kernel(const StreamParams prm)
+{
+    constexpr int NWIN = kWinOf(K);
+    __shared__ uint4 stage[kNS * 2 * kStreamTPB];
+    if (*prm.fallback != 0) return; // the list overflowed: the chunk kernels redo the batch
+    const uint32_t n_groups = prm.fallback[1];
+    for (uint32_t g = blockIdx.x; g < n_groups; g += gridDim.x) {
+        const uint2 rj = prm.long_groups[g];
+        const uint64_t a = __ldg(prm.offsets + rj.x), e = __ldg(prm.offsets + rj.x + 1);
+        const uint64_t lim = e - (uint64_t)(K - 1);                     // one past the record's last k-mer start (e - a > K)
+        const uint64_t p0 = ((a >> 7) + (uint64_t)rj.y * kLongGroup + threadIdx.x) << 7;
+        uint32_t cnt = 0;
+        if (p0 < lim) {
+            const uint32_t *__restrict__ pw = prm.packed + (p0 >> 4);
+            const uint16_t *__restrict__ vw = prm.vmask + (p0 >> 4);
+            uint32_t W[NWIN];
+#pragma unroll
+            for (int i = 0; i < NWIN; ++i) W[i] = __ldg(pw + i);
+            QueryLane<K, M, S, H, kStreamTPB> ql;
+            ql.prologue(W, prm, stage);
+            uint32_t res = 0;
+            for (int b = 0; b < (int)(kLongChunk / 16); ++b) {
+                const uint32_t wnext = __ldg(pw + b + NWIN);
+                const uint32_t v16 = __ldg(vw + b);
+                uint32_t res16 = 0;
+                static_for<0, 16>([&](auto jc) {
+                    constexpr int J = decltype(jc)::value;
+                    if (ql.template step<J>(W, prm, stage) == 0) res16 |= 1u << J;
+                });
+                res16 &= ~v16; // a1: positions without a valid k-mer answer false
+#pragma unroll
+                for (int i = 0; i + 1 < NWIN; ++i) W[i] = W[i + 1];
+                W[NWIN - 1] = wnext;
+                res = (res >> 16) | (res16 << 16);
+                if (b & 1) {
+                    const uint64_t w0 = p0 + 32ull * (uint64_t)(b >> 1);   // first position of this bitmap word
+                    const uint64_t lo = a > w0 ? a : w0, hi = lim < w0 + 32 ? lim : w0 + 32;
+                    if (hi > lo) {
+                        const uint32_t n = (uint32_t)(hi - lo);
+                        const uint32_t word = res & ((n == 32 ? 0xFFFFFFFFu : ((1u << n) - 1u)) << (uint32_t)(lo - w0));
+                        if (word) atomicOr(prm.bitmap + (w0 >> 5), word);
+                        cnt += __popc(word);
+                    }
+                }
+            }
+            cp_async_wait<0>(); // look-ahead copies nobody reads: drained before the next group reuses the slots
+        }
+        if (prm.counts != nullptr && cnt != 0) atomicAdd(prm.counts + rj.x, cnt);
+    }
 }
 
 // =============================================================================================

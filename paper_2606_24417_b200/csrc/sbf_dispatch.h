@@ -16,6 +16,7 @@ struct KernelEntry {
     stream_launch_fn insert_tma; // run flush = one 32-byte TMA reduction (filters much larger than L2)
     stream_launch_fn query;
     stream_launch_fn query_rec; // record mode (one thread per record)
+    stream_launch_fn query_long; // the long records record mode listed (one thread per 128-position chunk)
 };
 
 template <int K, int M, int S, int H, int MODE>
@@ -40,10 +41,19 @@ cudaError_t launch_stream_rec(const StreamParams &prm, cudaStream_t stream)
     return cudaGetLastError();
 }
 
+template <int K, int M, int S, int H>
+cudaError_t launch_stream_long(const StreamParams &prm, cudaStream_t stream)
+{
+    if (prm.n_rec == 0 || prm.long_groups == nullptr) return cudaSuccess;
+    // the group count lives on the device: a fixed grid strides over the list (and exits at once when it is empty)
+    stream_long_kernel<K, M, S, H><<<148 * 4, kStreamTPB, 0, stream>>>(prm);
+    return cudaGetLastError();
+}
+
 #define SBF_ENTRY(K, M, S, H) \
     { K, M, S, H, &sbfk::launch_stream<K, M, S, H, sbfk::kModeInsert>, &sbfk::launch_stream<K, M, S, H, sbfk::kModeInsertTma>, \
       &sbfk::launch_stream<K, M, S, H, sbfk::kModeQuery>, \
-      &sbfk::launch_stream_rec<K, M, S, H> }
+      &sbfk::launch_stream_rec<K, M, S, H>, &sbfk::launch_stream_long<K, M, S, H> }
 
 // One table per translation unit (compiled in parallel); each registers itself when the library is loaded.
 void register_table(const KernelEntry *entries, int n); // sbf_api.cu
